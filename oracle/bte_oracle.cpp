@@ -1,0 +1,285 @@
+/*
+ * bte_oracle.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, obviously-correct CPU statement (fp64, straight loops) of the Crank-Nicolson + leap-frog
+ * time step of arxiv 1401.6047.  It is the oracle the CUDA path is compared with.
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may build,
+ * load or call it.  It shares no code, header, table or constant generator with the CUDA library under
+ * paper_1401_6047_b200/csrc and neither includes the other.
+ *
+ * The method is a time iteration, so the oracle is the algorithm step by step, in the paper's order
+ * and notation.  Each function cites the passage it follows; the readings taken where the paper is
+ * garbled or silent carry the tags (C1..C15) of DESIGN.md "Readings of the paper".
+ *
+ * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): closed form at B=0 for every (n,m,k), the
+ * Esaki-Tsu-type steady drift velocity, norm conservation, relaxation to f0, the B=0 mirror symmetry,
+ * the field-reversal mirror, E=0 stationarity of f0 with order-2 convergence, order-2 convergence in
+ * dt, the Tucker ac averages, a dense brute-force restatement on tiny grids, checkerboard independence
+ * and affinity.  Absolute values of configs 1-4 have no closed form and the paper prints none:
+ * for those "parity unpinned" beyond the invariants listed above.
+ *
+ * Build: g++ -std=c++17 -O2 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).
+ * -ffp-contract=off: no FMA contraction, every operation rounds once, in the order written.
+ */
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+const double PI = 3.14159265358979323846;
+
+struct Sim {
+    int N, M1;              /* rows n = 0..N (eq. 22), columns m = 0..M, M1 = M+1                       */
+    double dt;
+    double E_dc, E_omega, omega, B, mu, alpha, phiy_min, phiy_max, kappa_scale;
+    int64_t n_steps_total, avg_start_step;
+    double dphi;
+    std::vector<double> phi;            /* phi_y(m)                                                     */
+    std::vector<double> a0;             /* a_n^(0)(m), eq. (15)                                          */
+    std::vector<double> ha, hb, fa, fb; /* whole grid z_h and fractional grid z_f, eq. (39)-(41)         */
+    std::vector<double> sa, sb;         /* snapshot used only by the start-up step                       */
+    int64_t step;
+    double norm, v_dr, sum_v, sum_c, sum_s, window;
+    int threads;
+};
+
+inline size_t idx(const Sim* s, int n, int m) { return (size_t)n * (size_t)s->M1 + (size_t)m; }
+
+/* Boundary conditions (22)-(23): a = 0 outside n in [0..N], m in [0..M]; b = 0 outside n in [1..N],
+ * m in [0..M] (reading C3: b_0 == 0 because sin(0*phi_x) = 0).                                          */
+inline double rd_a(const Sim* s, const double* a, int n, int m) {
+    if (n < 0 || n > s->N || m < 0 || m >= s->M1) return 0.0;
+    return a[idx(s, n, m)];
+}
+inline double rd_b(const Sim* s, const double* b, int n, int m) {
+    if (n < 1 || n > s->N || m < 0 || m >= s->M1) return 0.0;
+    return b[idx(s, n, m)];
+}
+
+/* E(t) = E_dc + E_omega cos(omega t). */
+inline double field_E(const Sim* s, double t) { return s->E_dc + s->E_omega * std::cos(s->omega * t); }
+
+/*
+ * Operator T of eq. (38): advance grid X in place by `delta`, the derivative terms A, B of eq. (30)-(31)
+ * taken from grid S, the rotation term at time ta (explicit half) and tb (implicit half).
+ *   kappa   = kappa_scale * B * delta / (4 dphi)                eq. (30)-(31) prefactor, reading C4
+ *   nu, xi  = 1 +- delta/2                                      eq. (34)-(35)
+ *   mu^t    = n * beta^t_m * delta / 2, beta = E + B phi_y(m)   eq. (28)-(29)
+ *   g, h                                                       eq. (36)-(37)
+ *   a', b'                                                     eq. (32) and (33) with the sign of (33)
+ *                                                              corrected (reading C2: Cramer's rule on
+ *                                                              (24)+(26), (25)+(27))
+ * X and S must not alias (the start-up step passes a snapshot).
+ */
+void apply_T(const Sim* s, double delta, double* Xa, double* Xb, const double* Sa, const double* Sb,
+             double ta, double tb) {
+    const int N = s->N, M1 = s->M1;
+    const double kappa = s->kappa_scale * s->B * delta / (4.0 * s->dphi);
+    const double nu = 1.0 + delta / 2.0;
+    const double xi = 1.0 - delta / 2.0;
+    const double Ea = field_E(s, ta);
+    const double Eb = field_E(s, tb);
+#pragma omp parallel for schedule(static) num_threads(s->threads)
+    for (int n = 0; n <= N; ++n) {
+        for (int m = 0; m < M1; ++m) {
+            const double beta_a = Ea + s->B * s->phi[m];
+            const double beta_b = Eb + s->B * s->phi[m];
+            const double mu_a = n * beta_a * delta / 2.0;
+            const double mu_b = n * beta_b * delta / 2.0;
+            const double chi = (n == 1) ? 2.0 : 1.0; /* eq. (11) */
+            const double Bt = kappa * (rd_b(s, Sb, n + 1, m + 1) - rd_b(s, Sb, n + 1, m - 1) -
+                                       rd_b(s, Sb, n - 1, m + 1) + rd_b(s, Sb, n - 1, m - 1));
+            const double At = kappa * (chi * (rd_a(s, Sa, n - 1, m + 1) - rd_a(s, Sa, n - 1, m - 1)) -
+                                       rd_a(s, Sa, n + 1, m + 1) + rd_a(s, Sa, n + 1, m - 1));
+            const size_t i = idx(s, n, m);
+            const double a = Xa[i];
+            const double b = Xb[i];
+            const double g = a * xi - b * mu_a + Bt + s->a0[i] * delta;
+            const double h = b * xi + a * mu_a + At;
+            const double det = nu * nu + mu_b * mu_b;
+            Xa[i] = (g * nu - h * mu_b) / det;
+            Xb[i] = (n >= 1) ? (g * mu_b + h * nu) / det : 0.0;
+        }
+    }
+}
+
+/* phi_y lattice (reading C8) and equilibrium coefficients, eq. (15)-(16) with sigma(0) = 1/2,
+ * sigma(n>=1) = 1 (reading C1).  I_n(mu)/I_0(mu) from the C++17 library routine (reading C13).
+ * Values of the Gaussian factor below 1e-300 are set to 0 (input-recipe clamp, C19).        */
+void fill_equilibrium(Sim* s) {
+    const int N = s->N, M1 = s->M1, M = M1 - 1;
+    s->dphi = (s->phiy_max - s->phiy_min) / M;
+    s->phi.resize(M1);
+    for (int m = 0; m < M1; ++m)
+        s->phi[m] = 0.5 * (s->phiy_min + s->phiy_max) + (m - M / 2.0) * s->dphi;
+    const double i0 = std::cyl_bessel_i(0.0, s->mu);
+    const double pref = std::sqrt(s->mu / (2.0 * PI * s->alpha));
+    s->a0.assign((size_t)(N + 1) * M1, 0.0);
+    for (int n = 0; n <= N; ++n) {
+        const double r = std::cyl_bessel_i((double)n, s->mu) / i0;
+        const double c = (n == 0) ? (1.0 / (2.0 * PI)) * pref : (r / PI) * pref;
+        for (int m = 0; m < M1; ++m) {
+            double gm = std::exp(-s->mu * s->phi[m] * s->phi[m] / 2.0);
+            if (gm < 1e-300) gm = 0.0;
+            s->a0[idx(s, n, m)] = c * gm;
+        }
+    }
+}
+
+/* Observables on the whole grid: eq. (12) and eq. (20) by the rectangle rule (reading C10). */
+void reduce_observables(Sim* s) {
+    double sa = 0.0, sb = 0.0;
+    for (int m = 0; m < s->M1; ++m) sa += s->ha[idx(s, 0, m)];
+    if (s->N >= 1)
+        for (int m = 0; m < s->M1; ++m) sb += s->hb[idx(s, 1, m)];
+    s->norm = 2.0 * PI * std::sqrt(s->alpha) * s->dphi * sa;
+    s->v_dr = PI * std::sqrt(s->alpha) * s->dphi * sb;
+}
+
+} // namespace
+
+extern "C" {
+
+struct oracle_params {
+    double E_dc, E_omega, omega, B, mu, alpha, phiy_min, phiy_max, kappa_scale;
+    int64_t n_steps_total, avg_start_step;
+};
+
+struct oracle_obs {
+    int64_t step;
+    double t, norm, v_dr, sum_v_dt, sum_vcos_dt, sum_vsin_dt, window, edge_leak;
+};
+
+void* oracle_create(int32_t n_harm, int32_t n_phiy, double dt, const oracle_params* p, int32_t threads) {
+    if (n_harm < 1 || n_phiy < 3 || !(dt > 0) || !(p->mu > 0) || !(p->alpha > 0) ||
+        !(p->phiy_max > p->phiy_min))
+        return nullptr;
+    Sim* s = new Sim();
+    s->N = n_harm; s->M1 = n_phiy; s->dt = dt;
+    s->E_dc = p->E_dc; s->E_omega = p->E_omega; s->omega = p->omega; s->B = p->B; s->mu = p->mu;
+    s->alpha = p->alpha; s->phiy_min = p->phiy_min; s->phiy_max = p->phiy_max;
+    s->kappa_scale = p->kappa_scale;
+    s->n_steps_total = p->n_steps_total; s->avg_start_step = p->avg_start_step;
+    s->threads = threads > 0 ? threads : 1;
+    fill_equilibrium(s);
+    const size_t P = (size_t)(s->N + 1) * s->M1;
+    s->ha.assign(P, 0.0); s->hb.assign(P, 0.0); s->fa.assign(P, 0.0); s->fb.assign(P, 0.0);
+    s->step = 0; s->norm = s->v_dr = s->sum_v = s->sum_c = s->sum_s = s->window = 0.0;
+    return s;
+}
+
+void oracle_destroy(void* h) { delete (Sim*)h; }
+
+/* Initial condition a = a^(0), b = 0 and start-up of the fractional grid: z^{1/2} by
+ * (38) with time step dt/2 (reading C6: delta = dt/2 everywhere, stencil from z^0,
+ * field times 0 and dt/2).                                                                             */
+void oracle_init_equilibrium(void* h) {
+    Sim* s = (Sim*)h;
+    s->ha = s->a0;
+    std::fill(s->hb.begin(), s->hb.end(), 0.0);
+    s->fa = s->ha; s->fb = s->hb;
+    apply_T(s, s->dt / 2.0, s->fa.data(), s->fb.data(), s->ha.data(), s->hb.data(), 0.0, s->dt / 2.0);
+    s->step = 0; s->sum_v = s->sum_c = s->sum_s = s->window = 0.0;
+    reduce_observables(s);
+}
+
+/* Recompute the fractional grid from the current whole grid exactly as the start-up does, treating the
+ * current whole-grid state as z^0 at t = 0 (test helper for arbitrary initial states).                 */
+void oracle_startup_from_whole(void* h) {
+    Sim* s = (Sim*)h;
+    s->fa = s->ha; s->fb = s->hb;
+    apply_T(s, s->dt / 2.0, s->fa.data(), s->fb.data(), s->ha.data(), s->hb.data(), 0.0, s->dt / 2.0);
+    s->step = 0; s->sum_v = s->sum_c = s->sum_s = s->window = 0.0;
+    reduce_observables(s);
+}
+
+/* n_steps leap-frog steps, eq. (40)-(41): whole grid with the stencil of the fractional grid, then the
+ * fractional grid with the stencil of the NEW whole grid (reading C5).  Times are formed by
+ * multiplication, never accumulated (reading C14).  After each step the observables (12), (20) and,
+ * for steps k+1 > avg_start_step, the running sums of eq. (17) (reading C9).  v_trace / norm_trace are
+ * optional per-step outputs (length n_steps).                                                          */
+void oracle_step(void* h, int64_t n_steps, double* v_trace, double* norm_trace) {
+    Sim* s = (Sim*)h;
+    for (int64_t j = 0; j < n_steps; ++j) {
+        if (s->n_steps_total > 0 && s->step >= s->n_steps_total) {
+            if (v_trace) v_trace[j] = s->v_dr;
+            if (norm_trace) norm_trace[j] = s->norm;
+            continue;
+        }
+        const double k = (double)s->step;
+        apply_T(s, s->dt, s->ha.data(), s->hb.data(), s->fa.data(), s->fb.data(), k * s->dt,
+                (k + 1.0) * s->dt);
+        apply_T(s, s->dt, s->fa.data(), s->fb.data(), s->ha.data(), s->hb.data(), (k + 0.5) * s->dt,
+                (k + 1.5) * s->dt);
+        s->step += 1;
+        const double t = (double)s->step * s->dt;
+        reduce_observables(s);
+        if (s->step > s->avg_start_step) {
+            s->sum_v += s->v_dr * s->dt;
+            s->sum_c += s->v_dr * std::cos(s->omega * t) * s->dt;
+            s->sum_s += s->v_dr * std::sin(s->omega * t) * s->dt;
+            s->window += s->dt;
+        }
+        if (v_trace) v_trace[j] = s->v_dr;
+        if (norm_trace) norm_trace[j] = s->norm;
+    }
+}
+
+void oracle_observables(void* h, oracle_obs* o) {
+    Sim* s = (Sim*)h;
+    o->step = s->step;
+    o->t = (double)s->step * s->dt;
+    o->norm = s->norm; o->v_dr = s->v_dr;
+    o->sum_v_dt = s->sum_v; o->sum_vcos_dt = s->sum_c; o->sum_vsin_dt = s->sum_s; o->window = s->window;
+    o->edge_leak = (s->N >= 1) ? std::fabs(s->hb[idx(s, 1, 0)]) + std::fabs(s->hb[idx(s, 1, s->M1 - 1)])
+                               : 0.0;
+}
+
+/* grid: 0 = whole, 1 = fractional.  a, b: (N+1) x (M+1) row-major, m fastest. */
+void oracle_get_state(void* h, int32_t grid, double* a, double* b) {
+    Sim* s = (Sim*)h;
+    const size_t bytes = sizeof(double) * (size_t)(s->N + 1) * s->M1;
+    std::memcpy(a, grid == 0 ? s->ha.data() : s->fa.data(), bytes);
+    std::memcpy(b, grid == 0 ? s->hb.data() : s->fb.data(), bytes);
+}
+
+void oracle_set_state(void* h, int32_t grid, const double* a, const double* b) {
+    Sim* s = (Sim*)h;
+    const size_t bytes = sizeof(double) * (size_t)(s->N + 1) * s->M1;
+    std::memcpy(grid == 0 ? s->ha.data() : s->fa.data(), a, bytes);
+    std::memcpy(grid == 0 ? s->hb.data() : s->fb.data(), b, bytes);
+    if (grid == 0) reduce_observables(s);
+}
+
+void oracle_get_equilibrium(void* h, double* phi, double* a0) {
+    Sim* s = (Sim*)h;
+    std::memcpy(phi, s->phi.data(), sizeof(double) * s->M1);
+    std::memcpy(a0, s->a0.data(), sizeof(double) * (size_t)(s->N + 1) * s->M1);
+}
+
+/* One bare application of T (eq. 38) to grid `target` (0 whole, 1 fractional) with the stencil taken
+ * from the OTHER grid, time step delta, field times ta, tb.  Test hook for the brute-force,
+ * checkerboard and affinity pins.                                                                      */
+void oracle_apply_T(void* h, int32_t target, double delta, double ta, double tb) {
+    Sim* s = (Sim*)h;
+    if (target == 0)
+        apply_T(s, delta, s->ha.data(), s->hb.data(), s->fa.data(), s->fb.data(), ta, tb);
+    else
+        apply_T(s, delta, s->fa.data(), s->fb.data(), s->ha.data(), s->hb.data(), ta, tb);
+}
+
+int32_t oracle_max_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+} /* extern "C" */
