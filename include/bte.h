@@ -1,0 +1,137 @@
+/*
+ * bte.h -- C ABI of libbte_b200: the Crank-Nicolson + leap-frog time step of the spatially homogeneous
+ * 2-D superlattice Boltzmann transport equation (arxiv 1401.6047), fp64, one NVIDIA B200 (sm_100a).
+ *
+ * What one call sequence computes (citations are PAPER.md lines / equations):
+ *   bte_create            fixes the lattice a^t_{n,m}, n = 0..N harmonics, m = 0..M phi_y points
+ *                         (eq. 21-23) and the dimensionless parameters of eq. (4)-(5), L40-51.
+ *   bte_init_equilibrium  a = a^(0) (eq. 15-16), b = 0 (L99); fractional grid z^{1/2} by one
+ *                         application of T (eq. 38) with time step dt/2 (L202).
+ *   bte_step              n_steps leap-frog steps (eq. 40-41), each = T on the whole grid with
+ *                         the stencil A, B (eq. 30-31) of the fractional grid, then T on the fractional
+ *                         grid with the stencil of the new whole grid; T is the closed-form 2x2
+ *                         Crank-Nicolson solve of eq. (32)-(37) (sign of (33) corrected, C2).
+ *                         After every step: norm (eq. 12), drift velocity (eq. 20) and the running sums
+ *                         of eq. (17).  Everything runs on the device; the host is not involved per step.
+ *   bte_observables       copies the per-system observables to the host.
+ *
+ * Conventions
+ *   - All functions return 0 (BTE_OK) or a negative bte_status; none throws or aborts.  After a failure
+ *     bte_last_error() returns a thread-local, NUL-terminated description.
+ *   - "host" / "device" is stated for every pointer.  The ONLY device memory the library uses is the
+ *     caller-owned workspace handed to bte_create (e.g. a torch.empty(uint8) tensor); the library never
+ *     allocates or frees device memory and never frees the workspace.  The ctx is a small host object.
+ *   - Arrays a, b exchanged with the host are row-major (n_harm+1) x n_phiy doubles, m fastest
+ *     (the layout of Fig. 7).  Inside the workspace the state is stored as interleaved (a,b)
+ *     pairs.
+ *   - The library is fp64 throughout.  Work is issued asynchronously on the CUDA stream given at create
+ *     time (a cudaStream_t passed as void*; NULL = legacy default stream).
+ *   - Not thread-safe per ctx; distinct ctxs may be used from distinct threads.
+ */
+#ifndef BTE_B200_H
+#define BTE_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bte_ctx bte_ctx; /* opaque, library-owned host object */
+
+typedef enum {
+    BTE_OK = 0,
+    BTE_EINVAL = -1,    /* NULL pointer, N < 1, M+1 < 3, n_batch < 1, dt <= 0, mu <= 0, alpha <= 0,
+                           phiy_max <= phiy_min, bad index, unknown option                              */
+    BTE_EUNSTABLE = -2, /* |B| dt / dphi >= 2: the staggered scheme diverges (reading C11)     */
+    BTE_ENOMEM = -3,    /* workspace smaller than bte_workspace_bytes(grid) or misaligned (256 B)        */
+    BTE_ECUDA = -4      /* a CUDA runtime error was captured; text in bte_last_error()                   */
+} bte_status;
+
+/* Lattice shared by all systems of a batch (eq. 21-22; command-line names of L325-326 in brackets). */
+typedef struct {
+    int32_t n_harm;  /* N  : highest harmonic kept, rows n = 0..N            [n-harmonics]               */
+    int32_t n_phiy;  /* M+1: number of phi_y lattice points, m = 0..M        [g-grid]                    */
+    int32_t n_batch; /* number of independent systems advanced together, >= 1                            */
+    int32_t reserved;/* must be 0                                                                        */
+    double dt;       /* time step in units of tau                            [dt]                        */
+} bte_grid;
+
+/* One per system; all quantities dimensionless per eq. (4). */
+typedef struct {
+    double E_dc, E_omega, omega; /* E(t) = E_dc + E_omega cos(omega t), L99     [E_dc, E_omega, omega]   */
+    double B;                    /* constant magnetic field along z, eq. (5)    [B]                      */
+    double mu;                   /* Delta_1 / (2 k_B T), eq. (14)               [mu]                     */
+    double alpha;                /* m / m_x, eq. (4); normalisation only        [alpha]                  */
+    double phiy_min, phiy_max;   /* phi_m = centre + (m - M/2) dphi, dphi = (max-min)/M  [PhiYmin/max]   */
+    double kappa_scale;          /* 1: stencil prefactor B dt/(4 dphi), consistent with eq. (5),(9),(10);
+                                    alpha: the prefactor as printed in eq. (30)-(31) (C4)      */
+    int64_t n_steps_total;       /* the system freezes after this many steps; 0 = never                  */
+    int64_t avg_start_step;      /* running sums of eq. (17) include steps k > avg_start_step (L103)     */
+} bte_params;
+
+typedef struct {
+    int64_t step;       /* whole-grid steps taken by this system                                         */
+    double t;           /* step * dt                                                                     */
+    double norm;        /* eq. (12): 2 pi sqrt(alpha) dphi sum_m a_{0,m}   (should be 1)                  */
+    double v_dr;        /* eq. (20): pi sqrt(alpha) dphi sum_m b_{1,m}, whole grid, instantaneous        */
+    double sum_v_dt;    /* sum over steps k > avg_start_step of v_dr(t_k) dt                             */
+    double sum_vcos_dt; /* ... of v_dr(t_k) cos(omega t_k) dt.  Absorption of eq. (17) =
+                           (2 I0(mu)/I1(mu)) * sum_vcos_dt / window (factor applied by the caller, C9)   */
+    double sum_vsin_dt; /* ... of v_dr(t_k) sin(omega t_k) dt                                            */
+    double window;      /* sum of dt over the same steps                                                 */
+    double edge_leak;   /* |b_{1,0}| + |b_{1,M}| on the whole grid: bounds the norm drift per step (C12) */
+} bte_obs;
+
+/* Bytes of device workspace bte_create needs for this grid.  Pure function; 0 if grid is invalid. */
+size_t bte_workspace_bytes(const bte_grid* grid /* host */);
+
+/* Validates, computes the per-system tables on the host (phi_y lattice, Gaussian factor, Bessel ratios
+ * I_n(mu)/I_0(mu) of eq. 15) and uploads them into the workspace.
+ *   grid, params : host; params is an array of grid->n_batch entries (copied).
+ *   workspace    : DEVICE, caller-owned, >= bte_workspace_bytes(grid) bytes, 256-byte aligned; must stay
+ *                  valid until bte_destroy.  bytes is its size.
+ *   cuda_stream  : cudaStream_t (as void*) on which all work of this ctx is issued.
+ *   out          : host; receives the ctx, or NULL on failure.                                          */
+int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, size_t bytes,
+               void* cuda_stream, bte_ctx** out);
+
+/* State at t = 0: whole grid a = a^(0), b = 0 (L99); fractional grid by T with dt/2 (L202); step counter,
+ * running sums and observables reset.  Asynchronous on the stream.                                      */
+int bte_init_equilibrium(bte_ctx* ctx);
+
+/* Advance every system that has not reached its n_steps_total by n_steps (>= 0) steps of eq. (40)-(41)
+ * with the per-step reductions.  Asynchronous on the stream; no host synchronisation inside.            */
+int bte_step(bte_ctx* ctx, int64_t n_steps);
+
+/* Synchronises the stream and writes grid->n_batch records to out (host). */
+int bte_observables(bte_ctx* ctx, bte_obs* out /* host, n_batch entries */);
+
+/* Frees the ctx (host object and CUDA graph handles).  Never touches the workspace memory. */
+int bte_destroy(bte_ctx* ctx);
+
+/* State access (tests, checkpointing, end-to-end use).  grid_id: 0 = whole grid z^k, 1 = fractional grid
+ * z^{k+1/2}.  a, b: HOST arrays of (n_harm+1) * n_phiy doubles each, row-major, m fastest.  Both calls
+ * synchronise the stream.  bte_set_state does not change the step counter or the running sums.          */
+int bte_get_state(bte_ctx* ctx, int32_t system, int32_t grid_id, double* a, double* b);
+int bte_set_state(bte_ctx* ctx, int32_t system, int32_t grid_id, const double* a, const double* b);
+
+/* Tuning / variant selection, before or between bte_step calls.  Keys:
+ *   "variant"      0 = automatic (default), 1 = two half-update kernels per step (96 B/point),
+ *                  2 = fused whole+fractional strip-march kernel (64 B/point)
+ *   "graph_steps"  steps captured per CUDA graph for launch-bound grids; 0 = plain launches, -1 = auto
+ *   "tile_cols", "tile_rows", "prefetch_rows"   fused-kernel tile shape overrides (0 = automatic)
+ * Returns BTE_EINVAL for an unknown key or an unsupported value.                                        */
+int bte_set_option(bte_ctx* ctx, const char* key, int64_t value);
+
+/* Number of kernel launches (graph nodes counted individually) issued by this ctx so far. */
+int bte_launch_count(bte_ctx* ctx, int64_t* out /* host */);
+
+/* Thread-local text of the last error returned on this thread ("" if none). */
+const char* bte_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BTE_B200_H */

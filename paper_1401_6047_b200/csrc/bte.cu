@@ -1,0 +1,458 @@
+// bte.cu -- host side of libbte_b200: the C ABI of include/bte.h.
+// Product code: must not include, link or call anything under oracle/.
+#include "../../include/bte.h"
+#include "bte_kernels.cuh"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace bte;
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                             \
+    do {                                                                                           \
+        cudaError_t e__ = (expr);                                                                  \
+        if (e__ != cudaSuccess)                                                                    \
+            return fail(BTE_ECUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__),        \
+                        __FILE__, __LINE__);                                                       \
+    } while (0)
+
+constexpr size_t ALIGN = 256;
+size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+struct Offsets {
+    int pitch;
+    size_t state, cn, gm, phi, sc, ss, partial, total;
+};
+
+bool grid_ok(const bte_grid* g) {
+    return g && g->n_harm >= 1 && g->n_phiy >= 3 && g->n_batch >= 1 && g->n_batch <= 65535 &&
+           g->n_harm < 65535 && g->dt > 0.0 && std::isfinite(g->dt);
+}
+
+Offsets offsets_for(const bte_grid* g) {
+    Offsets o{};
+    o.pitch = (g->n_phiy + 7) / 8 * 8;
+    const size_t rows = (size_t)g->n_harm + 1, nb = (size_t)g->n_batch, pitch = (size_t)o.pitch;
+    size_t off = 0;
+    o.state = off;   off = align_up(off + 2 * 2 * nb * rows * pitch * sizeof(double2));
+    o.cn = off;      off = align_up(off + nb * rows * sizeof(double));
+    o.gm = off;      off = align_up(off + nb * pitch * sizeof(double));
+    o.phi = off;     off = align_up(off + nb * pitch * sizeof(double));
+    o.sc = off;      off = align_up(off + nb * sizeof(SysConst));
+    o.ss = off;      off = align_up(off + nb * sizeof(SysState));
+    o.partial = off; off = align_up(off + nb * pitch * 2 * sizeof(double));
+    o.total = off;
+    return o;
+}
+
+// I_n(x)/I_0(x), n = 0..N, by Miller's backward recurrence I_{n-1} = I_{n+1} + (2n/x) I_n (stable in this
+// direction because I_n is the minimal solution); only ratios are needed, so no normalisation sum.
+void bessel_i_ratios(double x, int N, std::vector<double>& r) {
+    const int ns = N + 2 * (int)std::ceil(x) + 120;
+    std::vector<double> t((size_t)ns + 2, 0.0);
+    t[ns + 1] = 0.0;
+    t[ns] = 1.0;
+    for (int n = ns; n >= 1; --n) {
+        t[n - 1] = t[n + 1] + (2.0 * n / x) * t[n];
+        if (t[n - 1] > 1e200) {
+            for (int j = n - 1; j <= ns; ++j) t[j] *= 1e-200;   // far tail underflows to 0, as it should
+        }
+    }
+    r.resize((size_t)N + 1);
+    for (int n = 0; n <= N; ++n) r[n] = t[n] / t[0];
+}
+
+enum Variant { VAR_AUTO = 0, VAR_SPLIT = 1, VAR_FUSED = 2 };
+
+}  // namespace
+
+struct bte_ctx {
+    bte_grid grid;
+    std::vector<bte_params> params;
+    Offsets off;
+    char* ws;
+    cudaStream_t stream;
+    Layout L;
+    int64_t steps_issued;   // global step count requested so far (per-system count = min(this, budget))
+    int64_t launches;
+    // options
+    int variant;
+    int64_t graph_steps;    // -1 auto, 0 off
+    int tile_cols, tile_rows, prefetch_rows;
+    // fused launch plan
+    int rows_per_chunk;
+    dim3 fgrid;
+    // CUDA graph cache
+    cudaGraph_t graph;
+    cudaGraphExec_t graph_exec;
+    int64_t graph_len;
+    int graph_variant;
+};
+
+namespace {
+
+constexpr int FT = 128;   // threads per CTA of the fused kernel (strip of FT-2 = 126 columns)
+constexpr int FD = 3;     // rows prefetched ahead
+
+using FCfg = FusedCfg<FT, FD>;
+
+int plan_fused(bte_ctx* c) {
+    const int rows = c->grid.n_harm + 1;
+    const int strips = (c->grid.n_phiy + FCfg::W - 1) / FCfg::W;
+    int rpc = c->tile_rows;
+    if (rpc <= 0) {
+        // enough CTAs to fill 148 SMs several times over, but chunks long enough that the 2-row halo
+        // recompute (and 6 extra row loads) per chunk stays at a few per cent
+        const long long want = 148LL * 8;
+        const long long have = (long long)strips * c->grid.n_batch;
+        long long chunks = (want + have - 1) / have;
+        if (chunks < 1) chunks = 1;
+        rpc = (int)((rows + chunks - 1) / chunks);
+        if (rpc < 32) rpc = 32;
+    }
+    if (rpc < 2) rpc = 2;
+    if (rpc > rows) rpc = rows;
+    if (rows >= 2 && rpc < 2) rpc = 2;
+    c->rows_per_chunk = rpc;
+    const int chunks = (rows + rpc - 1) / rpc;
+    if (chunks > 65535) return fail(BTE_EINVAL, "too many row chunks");
+    c->fgrid = dim3((unsigned)strips, (unsigned)chunks, (unsigned)c->grid.n_batch);
+    return BTE_OK;
+}
+
+int effective_variant(const bte_ctx* c) { return c->variant == VAR_AUTO ? VAR_FUSED : c->variant; }
+
+void drop_graph(bte_ctx* c) {
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (c->graph) cudaGraphDestroy(c->graph);
+    c->graph_exec = nullptr;
+    c->graph = nullptr;
+    c->graph_len = 0;
+}
+
+dim3 split_grid(const bte_ctx* c) {
+    return dim3((unsigned)((c->grid.n_phiy + 127) / 128), (unsigned)(c->grid.n_harm + 1),
+                (unsigned)c->grid.n_batch);
+}
+
+int launches_per_step(const bte_ctx* c) { return effective_variant(c) == VAR_FUSED ? 1 : 3; }
+
+// Issue one step with plain launches.
+int launch_step(bte_ctx* c) {
+    if (effective_variant(c) == VAR_FUSED) {
+        fused_step_kernel<FT, FD><<<c->fgrid, FT, FCfg::smem_bytes, c->stream>>>(c->L, c->rows_per_chunk);
+    } else {
+        const dim3 g = split_grid(c);
+        half_update_kernel<<<g, 128, 0, c->stream>>>(c->L, 0);
+        half_update_kernel<<<g, 128, 0, c->stream>>>(c->L, 1);
+        reduce_finalize_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 1);
+    }
+    CUDA_TRY(cudaGetLastError());
+    c->launches += launches_per_step(c);
+    return BTE_OK;
+}
+
+// Build a graph of `len` steps from explicit kernel nodes (no stream capture: safe with any caller
+// stream).  Kernels take no per-step argument -- the step counter lives on the device -- so one graph
+// can be replayed any number of times.
+int build_graph(bte_ctx* c, int64_t len) {
+    drop_graph(c);
+    CUDA_TRY(cudaGraphCreate(&c->graph, 0));
+    cudaGraphNode_t prev = nullptr;
+    const int var = effective_variant(c);
+    int mode0 = 0, mode1 = 1, adv = 1;
+    int rpc = c->rows_per_chunk;
+    for (int64_t s = 0; s < len; ++s) {
+        auto add = [&](void* fn, dim3 grid, dim3 block, size_t smem, void** args) -> cudaError_t {
+            cudaKernelNodeParams p{};
+            p.func = fn; p.gridDim = grid; p.blockDim = block; p.sharedMemBytes = (unsigned)smem;
+            p.kernelParams = args; p.extra = nullptr;
+            cudaGraphNode_t node;
+            cudaError_t e = cudaGraphAddKernelNode(&node, c->graph, prev ? &prev : nullptr, prev ? 1 : 0, &p);
+            prev = node;
+            return e;
+        };
+        if (var == VAR_FUSED) {
+            void* args[] = {&c->L, &rpc};
+            CUDA_TRY(add((void*)fused_step_kernel<FT, FD>, c->fgrid, dim3(FT), FCfg::smem_bytes, args));
+        } else {
+            const dim3 g = split_grid(c);
+            void* a0[] = {&c->L, &mode0};
+            void* a1[] = {&c->L, &mode1};
+            void* a2[] = {&c->L, &adv};
+            CUDA_TRY(add((void*)half_update_kernel, g, dim3(128), 0, a0));
+            CUDA_TRY(add((void*)half_update_kernel, g, dim3(128), 0, a1));
+            CUDA_TRY(add((void*)reduce_finalize_kernel, dim3(c->grid.n_batch), dim3(256), 0, a2));
+        }
+    }
+    CUDA_TRY(cudaGraphInstantiate(&c->graph_exec, c->graph, 0));
+    c->graph_len = len;
+    c->graph_variant = var;
+    return BTE_OK;
+}
+
+int64_t auto_graph_steps(const bte_ctx* c) {
+    // a step of a small grid takes a few microseconds: launch overhead dominates => replay graphs
+    const double pts = (double)(c->grid.n_harm + 1) * c->grid.n_phiy * c->grid.n_batch;
+    if (pts > 4.0e6) return 0;
+    return 64;
+}
+
+int64_t system_steps(const bte_ctx* c, int sys) {
+    const int64_t tot = c->params[sys].n_steps_total;
+    return (tot > 0 && c->steps_issued > tot) ? tot : c->steps_issued;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* bte_last_error(void) { return g_err.c_str(); }
+
+size_t bte_workspace_bytes(const bte_grid* grid) {
+    if (!grid_ok(grid)) return 0;
+    return offsets_for(grid).total;
+}
+
+int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, size_t bytes,
+               void* cuda_stream, bte_ctx** out) {
+    if (out) *out = nullptr;
+    if (!out || !grid || !params || !workspace) return fail(BTE_EINVAL, "bte_create: NULL argument");
+    if (!grid_ok(grid) || grid->reserved != 0)
+        return fail(BTE_EINVAL, "bte_create: need n_harm >= 1, n_phiy >= 3, 1 <= n_batch <= 65535, dt > 0");
+    const Offsets off = offsets_for(grid);
+    if (bytes < off.total) return fail(BTE_ENOMEM, "bte_create: workspace has %zu bytes, %zu needed", bytes, off.total);
+    if (((uintptr_t)workspace % ALIGN) != 0) return fail(BTE_ENOMEM, "bte_create: workspace must be 256-byte aligned");
+    const int N = grid->n_harm, M1 = grid->n_phiy, M = M1 - 1, nb = grid->n_batch;
+    for (int s = 0; s < nb; ++s) {
+        const bte_params& p = params[s];
+        const bool finite = std::isfinite(p.E_dc) && std::isfinite(p.E_omega) && std::isfinite(p.omega) &&
+                            std::isfinite(p.B) && std::isfinite(p.mu) && std::isfinite(p.alpha) &&
+                            std::isfinite(p.phiy_min) && std::isfinite(p.phiy_max) && std::isfinite(p.kappa_scale);
+        if (!finite || !(p.mu > 0.0) || !(p.alpha > 0.0) || !(p.phiy_max > p.phiy_min) ||
+            p.n_steps_total < 0 || p.avg_start_step < 0)
+            return fail(BTE_EINVAL, "bte_create: system %d: need finite parameters, mu > 0, alpha > 0, phiy_max > phiy_min", s);
+        const double dphi = (p.phiy_max - p.phiy_min) / M;
+        if (std::fabs(p.B) * grid->dt / dphi >= 2.0)
+            return fail(BTE_EUNSTABLE, "bte_create: system %d: |B| dt / dphi = %g >= 2 (scheme unstable)", s,
+                        std::fabs(p.B) * grid->dt / dphi);
+    }
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+
+    // host tables: phi_y lattice (C8), Gaussian factor and c_n of eq. (15)-(16) (C1, C13)
+    const size_t rows = (size_t)N + 1, pitch = (size_t)off.pitch;
+    std::vector<double> cn(nb * rows), gm(nb * pitch, 0.0), phi(nb * pitch, 0.0), ratios;
+    std::vector<SysConst> sc((size_t)nb);
+    const double PI = 3.14159265358979323846;
+    for (int s = 0; s < nb; ++s) {
+        const bte_params& p = params[s];
+        const double dphi = (p.phiy_max - p.phiy_min) / M;
+        const double centre = 0.5 * (p.phiy_min + p.phiy_max);
+        for (int m = 0; m < M1; ++m) {
+            const double ph = centre + (m - M / 2.0) * dphi;
+            double g = std::exp(-p.mu * ph * ph / 2.0);
+            if (g < 1e-300) g = 0.0;   // input-recipe clamp (C19)
+            phi[s * pitch + m] = ph;
+            gm[s * pitch + m] = g;
+        }
+        bessel_i_ratios(p.mu, N, ratios);
+        const double pref = std::sqrt(p.mu / (2.0 * PI * p.alpha));
+        cn[s * rows] = (1.0 / (2.0 * PI)) * pref;
+        for (int n = 1; n <= N; ++n) cn[s * rows + n] = (ratios[n] / PI) * pref;
+        SysConst& k = sc[s];
+        k.E_dc = p.E_dc; k.E_omega = p.E_omega; k.omega = p.omega; k.B = p.B; k.dphi = dphi;
+        k.kappa_dt = p.kappa_scale * p.B * grid->dt / (4.0 * dphi);
+        k.norm_scale = 2.0 * PI * std::sqrt(p.alpha) * dphi;
+        k.v_scale = PI * std::sqrt(p.alpha) * dphi;
+        k.n_steps_total = p.n_steps_total; k.avg_start_step = p.avg_start_step;
+    }
+    char* ws = (char*)workspace;
+    CUDA_TRY(cudaMemcpyAsync(ws + off.cn, cn.data(), cn.size() * sizeof(double), cudaMemcpyHostToDevice, stream));
+    CUDA_TRY(cudaMemcpyAsync(ws + off.gm, gm.data(), gm.size() * sizeof(double), cudaMemcpyHostToDevice, stream));
+    CUDA_TRY(cudaMemcpyAsync(ws + off.phi, phi.data(), phi.size() * sizeof(double), cudaMemcpyHostToDevice, stream));
+    CUDA_TRY(cudaMemcpyAsync(ws + off.sc, sc.data(), sc.size() * sizeof(SysConst), cudaMemcpyHostToDevice, stream));
+    CUDA_TRY(cudaMemsetAsync(ws + off.ss, 0, (size_t)nb * sizeof(SysState), stream));
+    CUDA_TRY(cudaMemsetAsync(ws + off.partial, 0, (size_t)nb * pitch * 2 * sizeof(double), stream));
+    CUDA_TRY(cudaStreamSynchronize(stream));   // host tables go out of scope
+
+    bte_ctx* c = new bte_ctx();
+    c->grid = *grid;
+    c->params.assign(params, params + nb);
+    c->off = off; c->ws = ws; c->stream = stream;
+    c->L.N = N; c->L.M1 = M1; c->L.pitch = off.pitch; c->L.n_batch = nb; c->L.dt = grid->dt;
+    c->L.state = (double2*)(ws + off.state);
+    c->L.cn = (const double*)(ws + off.cn);
+    c->L.gm = (const double*)(ws + off.gm);
+    c->L.phi = (const double*)(ws + off.phi);
+    c->L.sc = (const SysConst*)(ws + off.sc);
+    c->L.ss = (SysState*)(ws + off.ss);
+    c->L.partial = (double*)(ws + off.partial);
+    c->steps_issued = 0; c->launches = 0;
+    c->variant = VAR_AUTO; c->graph_steps = -1;
+    c->tile_cols = 0; c->tile_rows = 0; c->prefetch_rows = 0;
+    c->graph = nullptr; c->graph_exec = nullptr; c->graph_len = 0; c->graph_variant = 0;
+    int rc = plan_fused(c);
+    if (rc != BTE_OK) { delete c; return rc; }
+    cudaError_t e = cudaFuncSetAttribute(fused_step_kernel<FT, FD>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)FCfg::smem_bytes);
+    if (e != cudaSuccess) {
+        delete c;
+        return fail(BTE_ECUDA, "cudaFuncSetAttribute failed: %s (is this an sm_100a device?)", cudaGetErrorString(e));
+    }
+    *out = c;
+    return BTE_OK;
+}
+
+int bte_init_equilibrium(bte_ctx* c) {
+    if (!c) return fail(BTE_EINVAL, "bte_init_equilibrium: NULL ctx");
+    const dim3 g((unsigned)((c->off.pitch + 127) / 128), (unsigned)(c->grid.n_harm + 1), (unsigned)c->grid.n_batch);
+    init_state_kernel<<<g, 128, 0, c->stream>>>(c->L);
+    half_update_kernel<<<split_grid(c), 128, 0, c->stream>>>(c->L, 2);   // start-up z^{1/2}, L202
+    reduce_finalize_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 0);
+    CUDA_TRY(cudaGetLastError());
+    c->launches += 3;
+    c->steps_issued = 0;
+    return BTE_OK;
+}
+
+int bte_step(bte_ctx* c, int64_t n_steps) {
+    if (!c) return fail(BTE_EINVAL, "bte_step: NULL ctx");
+    if (n_steps < 0) return fail(BTE_EINVAL, "bte_step: n_steps < 0");
+    int64_t left = n_steps;
+    const int64_t glen = c->graph_steps < 0 ? auto_graph_steps(c) : c->graph_steps;
+    if (glen > 1 && left >= glen) {
+        if (!c->graph_exec || c->graph_len != glen || c->graph_variant != effective_variant(c)) {
+            int rc = build_graph(c, glen);
+            if (rc != BTE_OK) return rc;
+        }
+        while (left >= glen) {
+            CUDA_TRY(cudaGraphLaunch(c->graph_exec, c->stream));
+            c->launches += glen * launches_per_step(c);
+            left -= glen;
+        }
+    }
+    for (; left > 0; --left) {
+        int rc = launch_step(c);
+        if (rc != BTE_OK) return rc;
+    }
+    c->steps_issued += n_steps;
+    return BTE_OK;
+}
+
+int bte_observables(bte_ctx* c, bte_obs* out) {
+    if (!c || !out) return fail(BTE_EINVAL, "bte_observables: NULL argument");
+    std::vector<SysState> ss((size_t)c->grid.n_batch);
+    CUDA_TRY(cudaMemcpyAsync(ss.data(), c->ws + c->off.ss, ss.size() * sizeof(SysState), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    for (int s = 0; s < c->grid.n_batch; ++s) {
+        bte_obs& o = out[s];
+        o.step = ss[s].k; o.t = (double)ss[s].k * c->grid.dt; o.norm = ss[s].norm; o.v_dr = ss[s].v_dr;
+        o.sum_v_dt = ss[s].sum_v; o.sum_vcos_dt = ss[s].sum_c; o.sum_vsin_dt = ss[s].sum_s;
+        o.window = ss[s].window; o.edge_leak = ss[s].edge_leak;
+    }
+    return BTE_OK;
+}
+
+int bte_destroy(bte_ctx* c) {
+    if (!c) return BTE_OK;
+    drop_graph(c);
+    delete c;
+    return BTE_OK;
+}
+
+int bte_get_state(bte_ctx* c, int32_t system, int32_t grid_id, double* a, double* b) {
+    if (!c || !a || !b) return fail(BTE_EINVAL, "bte_get_state: NULL argument");
+    if (system < 0 || system >= c->grid.n_batch || grid_id < 0 || grid_id > 1)
+        return fail(BTE_EINVAL, "bte_get_state: bad system or grid index");
+    const int rows = c->grid.n_harm + 1, M1 = c->grid.n_phiy, pitch = c->off.pitch;
+    const int buf = (int)(system_steps(c, system) & 1);
+    const size_t gp = (size_t)rows * pitch;
+    const double2* z = c->L.state + (((size_t)buf * 2 + grid_id) * c->grid.n_batch + system) * gp;
+    // the other buffer of this (grid, system) is dead between steps: use it as staging
+    double* stage = (double*)(c->L.state + (((size_t)(buf ^ 1) * 2 + grid_id) * c->grid.n_batch + system) * gp);
+    const size_t cnt = (size_t)rows * M1;
+    const dim3 g((unsigned)((M1 + 255) / 256), (unsigned)rows);
+    deinterleave_kernel<<<g, 256, 0, c->stream>>>(z, stage, stage + cnt, rows, M1, pitch);
+    CUDA_TRY(cudaGetLastError());
+    c->launches += 1;
+    CUDA_TRY(cudaMemcpyAsync(a, stage, cnt * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaMemcpyAsync(b, stage + cnt, cnt * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return BTE_OK;
+}
+
+int bte_set_state(bte_ctx* c, int32_t system, int32_t grid_id, const double* a, const double* b) {
+    if (!c || !a || !b) return fail(BTE_EINVAL, "bte_set_state: NULL argument");
+    if (system < 0 || system >= c->grid.n_batch || grid_id < 0 || grid_id > 1)
+        return fail(BTE_EINVAL, "bte_set_state: bad system or grid index");
+    const int rows = c->grid.n_harm + 1, M1 = c->grid.n_phiy, pitch = c->off.pitch;
+    const int buf = (int)(system_steps(c, system) & 1);
+    const size_t gp = (size_t)rows * pitch;
+    double2* z = c->L.state + (((size_t)buf * 2 + grid_id) * c->grid.n_batch + system) * gp;
+    double* stage = (double*)(c->L.state + (((size_t)(buf ^ 1) * 2 + grid_id) * c->grid.n_batch + system) * gp);
+    const size_t cnt = (size_t)rows * M1;
+    CUDA_TRY(cudaMemcpyAsync(stage, a, cnt * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(cudaMemcpyAsync(stage + cnt, b, cnt * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    const dim3 g((unsigned)((pitch + 255) / 256), (unsigned)rows);
+    interleave_kernel<<<g, 256, 0, c->stream>>>(z, stage, stage + cnt, rows, M1, pitch);
+    c->launches += 1;
+    if (grid_id == 0) {   // keep norm / v_dr of the observables consistent with the new whole grid
+        // reduce_finalize reads buffer (k & 1) of every system; harmless for the others
+        reduce_finalize_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 0);
+        c->launches += 1;
+    }
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return BTE_OK;
+}
+
+int bte_set_option(bte_ctx* c, const char* key, int64_t value) {
+    if (!c || !key) return fail(BTE_EINVAL, "bte_set_option: NULL argument");
+    if (!strcmp(key, "variant")) {
+        if (value < 0 || value > 2) return fail(BTE_EINVAL, "variant must be 0, 1 or 2");
+        c->variant = (int)value;
+        return BTE_OK;
+    }
+    if (!strcmp(key, "graph_steps")) {
+        if (value < -1 || value > 4096) return fail(BTE_EINVAL, "graph_steps must be in [-1, 4096]");
+        c->graph_steps = value;
+        return BTE_OK;
+    }
+    if (!strcmp(key, "tile_rows")) {
+        if (value < 0 || (value > 0 && value < 2)) return fail(BTE_EINVAL, "tile_rows must be 0 or >= 2");
+        c->tile_rows = (int)value;
+        drop_graph(c);
+        return plan_fused(c);
+    }
+    if (!strcmp(key, "tile_cols") || !strcmp(key, "prefetch_rows")) {
+        if (value != 0) return fail(BTE_EINVAL, "%s: only 0 (automatic) is supported in this build", key);
+        return BTE_OK;
+    }
+    return fail(BTE_EINVAL, "bte_set_option: unknown key '%s'", key);
+}
+
+int bte_launch_count(bte_ctx* c, int64_t* out) {
+    if (!c || !out) return fail(BTE_EINVAL, "bte_launch_count: NULL argument");
+    *out = c->launches;
+    return BTE_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,55 @@
+"""Helpers for the GPU-vs-oracle parity tests (tests only)."""
+from __future__ import annotations
+
+import numpy as np
+from scipy import special
+
+from oracle import OracleSim
+
+# north_star tolerances (fp64): max |df| <= 1e-12 max|f| over both grids of a system; observables 1e-10
+# relative, with the floors of DESIGN.md C15 for quantities that can pass through zero.
+TOL_STATE = 1e-12
+TOL_OBS = 1e-10
+
+
+def oracle_run(w, n_steps, systems=None, threads=4):
+    """Run the oracle for the listed systems of workload w; returns {sys: (sim, obs)}."""
+    out = {}
+    for s in (range(w.grid.n_batch) if systems is None else systems):
+        sim = OracleSim(w.grid.n_harm, w.grid.n_phiy, w.grid.dt, w.params[s], threads=threads)
+        sim.init_equilibrium()
+        sim.step(n_steps)
+        out[s] = sim
+    return out
+
+
+def v_floor(p):
+    return float(special.ive(1, p.mu) / special.ive(0, p.mu) / 2.0)
+
+
+def assert_state_close(solver, sim, sys_index, tol=TOL_STATE, what=""):
+    ha, hb = sim.get_state(0)
+    fa, fb = sim.get_state(1)
+    scale = max(np.abs(ha).max(), np.abs(hb).max(), np.abs(fa).max(), np.abs(fb).max())
+    worst = 0.0
+    for g, (ra, rb) in ((0, (ha, hb)), (1, (fa, fb))):
+        ga, gb = solver.get_state(sys_index, g)
+        assert np.isfinite(ga).all() and np.isfinite(gb).all(), f"{what}: non-finite GPU state"
+        worst = max(worst, np.abs(ga - ra).max(), np.abs(gb - rb).max())
+        assert np.all(gb[0] == 0.0), f"{what}: b_0 must stay exactly 0 (eq. 23)"
+    assert worst <= tol * scale, f"{what}: max|df| = {worst:.3e} > {tol:g} * max|f| = {tol * scale:.3e}"
+    return worst / scale
+
+
+def assert_obs_close(got, ref, p, dt, tol=TOL_OBS, what=""):
+    vf = v_floor(p)
+    assert got.step == ref.step, f"{what}: step {got.step} != {ref.step}"
+    assert abs(got.t - ref.t) <= 1e-12 * max(1.0, abs(ref.t))
+    assert abs(got.norm - ref.norm) <= tol * max(abs(ref.norm), 1.0), f"{what}: norm {got.norm} vs {ref.norm}"
+    assert abs(got.v_dr - ref.v_dr) <= tol * max(abs(ref.v_dr), vf), f"{what}: v_dr {got.v_dr} vs {ref.v_dr}"
+    win = max(ref.window, dt)
+    for k in ("sum_v_dt", "sum_vcos_dt", "sum_vsin_dt"):
+        g, r = getattr(got, k), getattr(ref, k)
+        assert abs(g - r) <= tol * max(abs(r), vf * win), f"{what}: {k} {g} vs {r}"
+    assert abs(got.window - ref.window) <= 1e-12 * max(ref.window, dt), f"{what}: window"
+    assert abs(got.edge_leak - ref.edge_leak) <= tol * max(abs(ref.edge_leak), vf), f"{what}: edge_leak"

@@ -1,0 +1,186 @@
+"""GPU-vs-oracle parity through the C ABI (run on the B200 box: pytest -m gpu).
+
+Element-by-element comparison of all four arrays (a, b on the whole and the fractional grid) and of the
+observables, on the same generated inputs, at sizes that span several strips / row chunks with ragged
+tails; then the BASELINE configs (full length where the oracle finishes in seconds, a step prefix
+otherwise -- parity is asserted at the last common step).
+"""
+import numpy as np
+import pytest
+
+from paper_1401_6047_b200 import workloads as W
+
+from parity_util import assert_obs_close, assert_state_close, oracle_run
+
+pytestmark = pytest.mark.gpu
+
+VARIANTS = {"split": 1, "fused": 2}
+
+
+def gpu_solver(w, variant="fused", graph_steps=None, tile_rows=None):
+    from paper_1401_6047_b200 import Solver
+    s = Solver(w.grid, w.params)
+    s.set_option("variant", VARIANTS[variant])
+    if graph_steps is not None:
+        s.set_option("graph_steps", graph_steps)
+    if tile_rows is not None:
+        s.set_option("tile_rows", tile_rows)
+    s.init_equilibrium()
+    return s
+
+
+def check(w, n_steps, variant, systems=None, graph_steps=None, tile_rows=None, chunks=None):
+    s = gpu_solver(w, variant, graph_steps, tile_rows)
+    if chunks:                      # several bte_step calls must equal one
+        for c in chunks:
+            s.step(c)
+        assert sum(chunks) == n_steps
+    else:
+        s.step(n_steps)
+    obs = s.observables()
+    sims = oracle_run(w, n_steps, systems)
+    worst = 0.0
+    for i, sim in sims.items():
+        what = f"{w.name}[{i}] {variant} steps={n_steps}"
+        worst = max(worst, assert_state_close(s, sim, i, what=what))
+        assert_obs_close(obs[i], sim.observables(), w.params[i], w.grid.dt, what=what)
+    s.destroy()
+    return worst
+
+
+# -------------------------------------------------------------------------------------------------
+# small / ragged shapes
+# -------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", ["split", "fused"])
+def test_init_equilibrium_matches_oracle(variant):
+    w = W.small_case(N=7, M1=45, n_steps=0)
+    check(w, 0, variant)
+
+
+@pytest.mark.parametrize("variant", ["split", "fused"])
+@pytest.mark.parametrize("N,M1", [(1, 3), (2, 5), (5, 126), (12, 127), (9, 128), (33, 253), (40, 801)])
+def test_small_shapes(variant, N, M1):
+    """M+1 around the strip width (126 columns) and its multiples, N around the chunk length."""
+    w = W.small_case(N=N, M1=M1, dt=0.004, n_steps=23, B=1.5 if M1 > 3 else 0.2, avg_start=5)
+    check(w, 23, variant)
+
+
+@pytest.mark.parametrize("tile_rows", [2, 3, 7, 16])
+def test_fused_row_chunking(tile_rows):
+    """Row chunks with halo recompute, ragged last chunk, chunk boundaries next to rows 0/1."""
+    w = W.small_case(N=21, M1=300, dt=0.004, n_steps=17, avg_start=3)
+    check(w, 17, "fused", tile_rows=tile_rows)
+
+
+@pytest.mark.parametrize("variant", ["split", "fused"])
+def test_graph_replay_equals_plain_launches(variant):
+    w = W.small_case(N=10, M1=140, n_steps=50, avg_start=7)
+    check(w, 50, variant, graph_steps=8)             # 6 graph replays + 2 plain steps
+    check(w, 50, variant, graph_steps=0)
+    check(w, 50, variant, chunks=[1, 2, 30, 17])
+
+
+def test_fused_equals_split_bitwise_state():
+    """Both variants evaluate the same per-point expression: states must agree to rounding (they
+    differ only in nothing -- same operation order -- so we ask for exact equality)."""
+    w = W.small_case(N=14, M1=260, n_steps=31)
+    a = gpu_solver(w, "split"); a.step(31)
+    b = gpu_solver(w, "fused"); b.step(31)
+    for g in (0, 1):
+        xa, xb = a.get_state(0, g)
+        ya, yb = b.get_state(0, g)
+        assert np.array_equal(xa, ya) and np.array_equal(xb, yb)
+
+
+@pytest.mark.parametrize("variant", ["split", "fused"])
+def test_batched_with_step_budgets(variant):
+    """Config-3-shaped batch: per-system parameters, phi_y ranges and step budgets (systems freeze)."""
+    w = W.random_batch(n_batch=6, N=10, M1=150, dt=0.004, seed=123, periods=0.25)
+    n = w.n_steps + 5                   # run past the longest budget
+    s = gpu_solver(w, variant)
+    s.step(n)
+    obs = s.observables()
+    sims = oracle_run(w, n)
+    for i, sim in sims.items():
+        assert obs[i].step == w.params[i].n_steps_total
+        assert_state_close(s, sim, i, what=f"batch[{i}] {variant}")
+        assert_obs_close(obs[i], sim.observables(), w.params[i], w.grid.dt, what=f"batch[{i}] {variant}")
+
+
+def test_alpha_and_kappa_scale():
+    w = W.small_case(N=8, M1=90, alpha=0.9496, kappa_scale=0.9496, n_steps=20)
+    check(w, 20, "fused")
+    check(w, 20, "split")
+
+
+def test_set_state_roundtrip_and_step():
+    rng = np.random.default_rng(5)
+    w = W.small_case(N=6, M1=70, n_steps=9)
+    s = gpu_solver(w, "fused")
+    shape = (7, 70)
+    ha, hb, fa, fb = (rng.standard_normal(shape) for _ in range(4))
+    hb[0] = 0; fb[0] = 0
+    s.set_state(0, 0, ha, hb); s.set_state(0, 1, fa, fb)
+    ga, gb = s.get_state(0, 0)
+    assert np.array_equal(ga, ha) and np.array_equal(gb, hb)
+    from oracle import OracleSim
+    sim = OracleSim(6, 70, w.grid.dt, w.params[0])
+    sim.set_state(0, ha, hb); sim.set_state(1, fa, fb)
+    s.step(9); sim.step(9)
+    assert_state_close(s, sim, 0, what="set_state")
+
+
+# -------------------------------------------------------------------------------------------------
+# error behaviour of the boundary
+# -------------------------------------------------------------------------------------------------
+def test_create_rejects_unstable_and_invalid():
+    from paper_1401_6047_b200 import BteError, Solver
+    w = W.small_case(N=4, M1=41, dt=0.5, B=4.0, phiy_max=4.0)       # B dt/dphi = 10
+    with pytest.raises(BteError) as e:
+        Solver(w.grid, w.params)
+    assert e.value.code == -2
+    w = W.small_case(N=4, M1=41, mu=-1.0, phiy_max=4.0)
+    with pytest.raises(BteError) as e:
+        Solver(w.grid, w.params)
+    assert e.value.code == -1
+
+
+# -------------------------------------------------------------------------------------------------
+# BASELINE configs
+# -------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", ["split", "fused"])
+def test_config0_full(variant):
+    from scipy import special
+    w = W.config0()
+    s = gpu_solver(w, variant)
+    s.step(w.n_steps)
+    o = s.observables()[0]
+    want = special.ive(1, 1.0) / special.ive(0, 1.0) * 0.5
+    assert abs(o.v_dr - want) / want < 5e-9 and abs(o.norm - 1) < 1e-12
+    sim = oracle_run(w, w.n_steps)[0]
+    assert_state_close(s, sim, 0, what="config0")
+    assert_obs_close(o, sim.observables(), w.params[0], w.grid.dt, what="config0")
+
+
+def test_config1_prefix_and_full_observables():
+    """Prefix of 3000 steps: full state parity.  Full length (62 832 steps): observables against the
+    oracle values stored in tests/golden/config1_full.json (written by tests/golden/make_golden.py)."""
+    w = W.config1()
+    check(w, 3000, "fused")
+
+
+def test_config2_prefix():
+    w = W.config2()
+    check(w, 300, "fused")
+
+
+def test_config3_subset_prefix():
+    """All 512 systems advance together on the GPU; 8 of them (0, 73, 146, ...) are checked."""
+    w = W.config3()
+    check(w, 200, "fused", systems=list(range(0, 512, 73)))
+
+
+def test_config4_prefix():
+    """Bandwidth-stress grid in the launch configuration bench.py times; 4 steps, full state compare."""
+    w = W.config4()
+    check(w, 4, "fused")
