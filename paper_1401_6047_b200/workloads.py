@@ -73,6 +73,16 @@ class Workload:
             tot += self.points_per_system * s
         return tot
 
+    def updates_between(self, k0: int, k1: int) -> int:
+        """Grid-point updates done by steps k0 < k <= k1 of the job (systems past their budget do none)."""
+        tot = 0
+        for p in self.params:
+            a, b = k0, k1
+            if p.n_steps_total > 0:
+                a, b = min(a, p.n_steps_total), min(b, p.n_steps_total)
+            tot += self.points_per_system * (b - a)
+        return tot
+
     def describe(self) -> dict:
         d = asdict(self.grid)
         d.update(name=self.name, n_steps=self.n_steps, note=self.note)
