@@ -1,7 +1,7 @@
 // bte.cu -- host side of libbte_b200: the C ABI of include/bte.h.
 // Product code: must not include, link or call anything under oracle/.
 #include "../../include/bte.h"
-#include "bte_kernels.cuh"
+#include "bte_fused_linear.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -39,7 +39,7 @@ size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Offsets {
     int pitch;
-    size_t state, cn, gm, phi, sc, ss, partial, total;
+    size_t state, state_bytes, cn, gm, phi, sc, ss, partial, gctl, total;
 };
 
 bool grid_ok(const bte_grid* g) {
@@ -50,15 +50,17 @@ bool grid_ok(const bte_grid* g) {
 Offsets offsets_for(const bte_grid* g) {
     Offsets o{};
     o.pitch = (g->n_phiy + 7) / 8 * 8;
-    const size_t rows = (size_t)g->n_harm + 1, nb = (size_t)g->n_batch, pitch = (size_t)o.pitch;
+    const size_t rows = (size_t)g->n_harm + 1 + 2 * GHOST, nb = (size_t)g->n_batch, pitch = (size_t)o.pitch;
     size_t off = 0;
     o.state = off;   off = align_up(off + 2 * 2 * nb * rows * pitch * sizeof(double2));
+    o.state_bytes = 2 * 2 * nb * rows * pitch * sizeof(double2);
     o.cn = off;      off = align_up(off + nb * rows * sizeof(double));
     o.gm = off;      off = align_up(off + nb * pitch * sizeof(double));
     o.phi = off;     off = align_up(off + nb * pitch * sizeof(double));
     o.sc = off;      off = align_up(off + nb * sizeof(SysConst));
     o.ss = off;      off = align_up(off + nb * sizeof(SysState));
     o.partial = off; off = align_up(off + nb * pitch * 2 * sizeof(double));
+    o.gctl = off;    off = align_up(off + 64);
     o.total = off;
     return o;
 }
@@ -80,7 +82,7 @@ void bessel_i_ratios(double x, int N, std::vector<double>& r) {
     for (int n = 0; n <= N; ++n) r[n] = t[n] / t[0];
 }
 
-enum Variant { VAR_AUTO = 0, VAR_SPLIT = 1, VAR_FUSED = 2 };
+enum Variant { VAR_AUTO = 0, VAR_SPLIT = 1, VAR_FUSED = 2, VAR_LINEAR = 3 };
 
 }  // namespace
 
@@ -97,9 +99,14 @@ struct bte_ctx {
     int variant;
     int64_t graph_steps;    // -1 auto, 0 off
     int tile_cols, tile_rows, prefetch_rows;
-    // fused launch plan
+    // fused (tile grid) launch plan
     int rows_per_chunk;
     dim3 fgrid;
+    // fused linear (persistent, one wave) launch plan
+    bool has_budgets;
+    int lin_grid;        // 0 = variant not usable for this problem
+    int lin_occ, sm_count;
+    int lin_minb;        // __launch_bounds__ min-blocks instantiation of the linear kernel (4, 5 or 6)
     // CUDA graph cache
     cudaGraph_t graph;
     cudaGraphExec_t graph_exec;
@@ -138,7 +145,49 @@ int plan_fused(bte_ctx* c) {
     return BTE_OK;
 }
 
-int effective_variant(const bte_ctx* c) { return c->variant == VAR_AUTO ? VAR_FUSED : c->variant; }
+using LCfg = LinCfg<FT>;
+
+void* linear_fn(const bte_ctx* c) {
+    if (c->lin_minb == 4)
+        return c->has_budgets ? (void*)fused_linear_kernel<FT, true, 4> : (void*)fused_linear_kernel<FT, false, 4>;
+    if (c->lin_minb == 6)
+        return c->has_budgets ? (void*)fused_linear_kernel<FT, true, 6> : (void*)fused_linear_kernel<FT, false, 6>;
+    return c->has_budgets ? (void*)fused_linear_kernel<FT, true, 5> : (void*)fused_linear_kernel<FT, false, 5>;
+}
+
+int plan_linear(bte_ctx* c) {
+    c->lin_grid = 0;
+    int dev = 0, sms = 0, occ = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    void* fn = linear_fn(c);
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LCfg::smem_bytes);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, FT, LCfg::smem_bytes);
+    if (e != cudaSuccess) return fail(BTE_ECUDA, "fused_linear_kernel setup failed: %s", cudaGetErrorString(e));
+    if (occ < 1) return BTE_OK;
+    c->lin_occ = occ; c->sm_count = sms;
+    const long long strips = (c->grid.n_phiy + LCfg::W - 1) / LCfg::W;
+    const long long rows_alloc = c->grid.n_harm + 1 + 2 * GHOST;
+    const long long units = strips * (c->grid.n_harm + 1) * (long long)c->grid.n_batch;
+    // 32-bit element offsets inside the kernel: both grids of one buffer, all systems
+    if (2LL * c->grid.n_batch * rows_alloc * c->off.pitch >= (1LL << 31)) return BTE_OK;
+    if (units >= (1LL << 31)) return BTE_OK;
+    long long g = (long long)sms * occ;
+    const long long min_rows = c->tile_cols > 0 ? 1 : 8;   // a CTA should own at least a few rows
+    if (c->tile_cols > 0) g = c->tile_cols;             // option "tile_cols" doubles as a grid-size override
+    if (g > (units + min_rows - 1) / min_rows) g = (units + min_rows - 1) / min_rows;
+    if (g < 1) g = 1;
+    // one CTA range may touch at most MAX_SPAN systems (shared-memory list)
+    if (c->has_budgets && (long long)c->grid.n_batch / g + 2 > LCfg::MAX_SPAN) return BTE_OK;
+    c->lin_grid = (int)g;
+    return BTE_OK;
+}
+
+int effective_variant(const bte_ctx* c) {
+    if (c->variant == VAR_AUTO) return c->lin_grid > 0 ? VAR_LINEAR : VAR_FUSED;
+    if (c->variant == VAR_LINEAR && c->lin_grid == 0) return VAR_FUSED;
+    return c->variant;
+}
 
 void drop_graph(bte_ctx* c) {
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
@@ -153,11 +202,15 @@ dim3 split_grid(const bte_ctx* c) {
                 (unsigned)c->grid.n_batch);
 }
 
-int launches_per_step(const bte_ctx* c) { return effective_variant(c) == VAR_FUSED ? 1 : 3; }
+int launches_per_step(const bte_ctx* c) { return effective_variant(c) == VAR_SPLIT ? 3 : 1; }
 
 // Issue one step with plain launches.
 int launch_step(bte_ctx* c) {
-    if (effective_variant(c) == VAR_FUSED) {
+    const int var = effective_variant(c);
+    if (var == VAR_LINEAR) {
+        void* args[] = {&c->L};
+        CUDA_TRY(cudaLaunchKernel(linear_fn(c), dim3(c->lin_grid), dim3(FT), args, LCfg::smem_bytes, c->stream));
+    } else if (var == VAR_FUSED) {
         fused_step_kernel<FT, FD><<<c->fgrid, FT, FCfg::smem_bytes, c->stream>>>(c->L, c->rows_per_chunk);
     } else {
         const dim3 g = split_grid(c);
@@ -190,7 +243,10 @@ int build_graph(bte_ctx* c, int64_t len) {
             prev = node;
             return e;
         };
-        if (var == VAR_FUSED) {
+        if (var == VAR_LINEAR) {
+            void* args[] = {&c->L};
+            CUDA_TRY(add(linear_fn(c), dim3(c->lin_grid), dim3(FT), LCfg::smem_bytes, args));
+        } else if (var == VAR_FUSED) {
             void* args[] = {&c->L, &rpc};
             CUDA_TRY(add((void*)fused_step_kernel<FT, FD>, c->fgrid, dim3(FT), FCfg::smem_bytes, args));
         } else {
@@ -239,6 +295,8 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
     if (!grid_ok(grid) || grid->reserved != 0)
         return fail(BTE_EINVAL, "bte_create: need n_harm >= 1, n_phiy >= 3, 1 <= n_batch <= 65535, dt > 0");
     const Offsets off = offsets_for(grid);
+    if (((long long)grid->n_harm + 1 + 2 * GHOST) * off.pitch >= (1LL << 31) - 8LL * off.pitch)
+        return fail(BTE_EINVAL, "bte_create: (n_harm+1) * n_phiy must stay below 2^31 points per system");
     if (bytes < off.total) return fail(BTE_ENOMEM, "bte_create: workspace has %zu bytes, %zu needed", bytes, off.total);
     if (((uintptr_t)workspace % ALIGN) != 0) return fail(BTE_ENOMEM, "bte_create: workspace must be 256-byte aligned");
     const int N = grid->n_harm, M1 = grid->n_phiy, M = M1 - 1, nb = grid->n_batch;
@@ -258,8 +316,8 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
     cudaStream_t stream = (cudaStream_t)cuda_stream;
 
     // host tables: phi_y lattice (C8), Gaussian factor and c_n of eq. (15)-(16) (C1, C13)
-    const size_t rows = (size_t)N + 1, pitch = (size_t)off.pitch;
-    std::vector<double> cn(nb * rows), gm(nb * pitch, 0.0), phi(nb * pitch, 0.0), ratios;
+    const size_t rows = (size_t)N + 1 + 2 * GHOST, pitch = (size_t)off.pitch;   // with ghost entries (zero)
+    std::vector<double> cn(nb * rows, 0.0), gm(nb * pitch, 0.0), phi(nb * pitch, 0.0), ratios;
     std::vector<SysConst> sc((size_t)nb);
     const double PI = 3.14159265358979323846;
     for (int s = 0; s < nb; ++s) {
@@ -275,8 +333,8 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
         }
         bessel_i_ratios(p.mu, N, ratios);
         const double pref = std::sqrt(p.mu / (2.0 * PI * p.alpha));
-        cn[s * rows] = (1.0 / (2.0 * PI)) * pref;
-        for (int n = 1; n <= N; ++n) cn[s * rows + n] = (ratios[n] / PI) * pref;
+        cn[s * rows + GHOST] = (1.0 / (2.0 * PI)) * pref;
+        for (int n = 1; n <= N; ++n) cn[s * rows + GHOST + n] = (ratios[n] / PI) * pref;
         SysConst& k = sc[s];
         k.E_dc = p.E_dc; k.E_omega = p.E_omega; k.omega = p.omega; k.B = p.B; k.dphi = dphi;
         k.kappa_dt = p.kappa_scale * p.B * grid->dt / (4.0 * dphi);
@@ -289,8 +347,10 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
     CUDA_TRY(cudaMemcpyAsync(ws + off.gm, gm.data(), gm.size() * sizeof(double), cudaMemcpyHostToDevice, stream));
     CUDA_TRY(cudaMemcpyAsync(ws + off.phi, phi.data(), phi.size() * sizeof(double), cudaMemcpyHostToDevice, stream));
     CUDA_TRY(cudaMemcpyAsync(ws + off.sc, sc.data(), sc.size() * sizeof(SysConst), cudaMemcpyHostToDevice, stream));
+    CUDA_TRY(cudaMemsetAsync(ws + off.state, 0, off.state_bytes, stream));   // ghost rows stay zero forever
     CUDA_TRY(cudaMemsetAsync(ws + off.ss, 0, (size_t)nb * sizeof(SysState), stream));
     CUDA_TRY(cudaMemsetAsync(ws + off.partial, 0, (size_t)nb * pitch * 2 * sizeof(double), stream));
+    CUDA_TRY(cudaMemsetAsync(ws + off.gctl, 0, 64, stream));
     CUDA_TRY(cudaStreamSynchronize(stream));   // host tables go out of scope
 
     bte_ctx* c = new bte_ctx();
@@ -298,6 +358,8 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
     c->params.assign(params, params + nb);
     c->off = off; c->ws = ws; c->stream = stream;
     c->L.N = N; c->L.M1 = M1; c->L.pitch = off.pitch; c->L.n_batch = nb; c->L.dt = grid->dt;
+    c->L.nu = 1.0 + 0.5 * grid->dt; c->L.xi = 1.0 - 0.5 * grid->dt; c->L.nu2 = c->L.nu * c->L.nu;
+    c->L.hd = 0.5 * grid->dt;
     c->L.state = (double2*)(ws + off.state);
     c->L.cn = (const double*)(ws + off.cn);
     c->L.gm = (const double*)(ws + off.gm);
@@ -305,6 +367,10 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
     c->L.sc = (const SysConst*)(ws + off.sc);
     c->L.ss = (SysState*)(ws + off.ss);
     c->L.partial = (double*)(ws + off.partial);
+    c->L.gctl = (unsigned int*)(ws + off.gctl);
+    c->has_budgets = false;
+    for (int s = 0; s < nb; ++s) c->has_budgets = c->has_budgets || params[s].n_steps_total > 0;
+    c->lin_grid = 0; c->lin_occ = 0; c->sm_count = 0; c->lin_minb = 4;
     c->steps_issued = 0; c->launches = 0;
     c->variant = VAR_AUTO; c->graph_steps = -1;
     c->tile_cols = 0; c->tile_rows = 0; c->prefetch_rows = 0;
@@ -317,6 +383,8 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
         delete c;
         return fail(BTE_ECUDA, "cudaFuncSetAttribute failed: %s (is this an sm_100a device?)", cudaGetErrorString(e));
     }
+    rc = plan_linear(c);
+    if (rc != BTE_OK) { delete c; return rc; }
     *out = c;
     return BTE_OK;
 }
@@ -384,10 +452,10 @@ int bte_get_state(bte_ctx* c, int32_t system, int32_t grid_id, double* a, double
         return fail(BTE_EINVAL, "bte_get_state: bad system or grid index");
     const int rows = c->grid.n_harm + 1, M1 = c->grid.n_phiy, pitch = c->off.pitch;
     const int buf = (int)(system_steps(c, system) & 1);
-    const size_t gp = (size_t)rows * pitch;
-    const double2* z = c->L.state + (((size_t)buf * 2 + grid_id) * c->grid.n_batch + system) * gp;
-    // the other buffer of this (grid, system) is dead between steps: use it as staging
-    double* stage = (double*)(c->L.state + (((size_t)(buf ^ 1) * 2 + grid_id) * c->grid.n_batch + system) * gp);
+    const size_t gp = (size_t)(rows + 2 * GHOST) * pitch, row0 = (size_t)GHOST * pitch;
+    const double2* z = c->L.state + (((size_t)buf * 2 + grid_id) * c->grid.n_batch + system) * gp + row0;
+    // rows 0..N of the other buffer of this (grid, system) are dead between steps: use them as staging
+    double* stage = (double*)(c->L.state + (((size_t)(buf ^ 1) * 2 + grid_id) * c->grid.n_batch + system) * gp + row0);
     const size_t cnt = (size_t)rows * M1;
     const dim3 g((unsigned)((M1 + 255) / 256), (unsigned)rows);
     deinterleave_kernel<<<g, 256, 0, c->stream>>>(z, stage, stage + cnt, rows, M1, pitch);
@@ -405,9 +473,9 @@ int bte_set_state(bte_ctx* c, int32_t system, int32_t grid_id, const double* a, 
         return fail(BTE_EINVAL, "bte_set_state: bad system or grid index");
     const int rows = c->grid.n_harm + 1, M1 = c->grid.n_phiy, pitch = c->off.pitch;
     const int buf = (int)(system_steps(c, system) & 1);
-    const size_t gp = (size_t)rows * pitch;
-    double2* z = c->L.state + (((size_t)buf * 2 + grid_id) * c->grid.n_batch + system) * gp;
-    double* stage = (double*)(c->L.state + (((size_t)(buf ^ 1) * 2 + grid_id) * c->grid.n_batch + system) * gp);
+    const size_t gp = (size_t)(rows + 2 * GHOST) * pitch, row0 = (size_t)GHOST * pitch;
+    double2* z = c->L.state + (((size_t)buf * 2 + grid_id) * c->grid.n_batch + system) * gp + row0;
+    double* stage = (double*)(c->L.state + (((size_t)(buf ^ 1) * 2 + grid_id) * c->grid.n_batch + system) * gp + row0);
     const size_t cnt = (size_t)rows * M1;
     CUDA_TRY(cudaMemcpyAsync(stage, a, cnt * sizeof(double), cudaMemcpyHostToDevice, c->stream));
     CUDA_TRY(cudaMemcpyAsync(stage + cnt, b, cnt * sizeof(double), cudaMemcpyHostToDevice, c->stream));
@@ -427,8 +495,9 @@ int bte_set_state(bte_ctx* c, int32_t system, int32_t grid_id, const double* a, 
 int bte_set_option(bte_ctx* c, const char* key, int64_t value) {
     if (!c || !key) return fail(BTE_EINVAL, "bte_set_option: NULL argument");
     if (!strcmp(key, "variant")) {
-        if (value < 0 || value > 2) return fail(BTE_EINVAL, "variant must be 0, 1 or 2");
+        if (value < 0 || value > 3) return fail(BTE_EINVAL, "variant must be 0, 1, 2 or 3");
         c->variant = (int)value;
+        drop_graph(c);
         return BTE_OK;
     }
     if (!strcmp(key, "graph_steps")) {
@@ -442,7 +511,19 @@ int bte_set_option(bte_ctx* c, const char* key, int64_t value) {
         drop_graph(c);
         return plan_fused(c);
     }
-    if (!strcmp(key, "tile_cols") || !strcmp(key, "prefetch_rows")) {
+    if (!strcmp(key, "tile_cols")) {   // CTAs of the persistent fused_linear_kernel (0 = SMs x occupancy)
+        if (value < 0 || value > 65535) return fail(BTE_EINVAL, "tile_cols must be in [0, 65535]");
+        c->tile_cols = (int)value;
+        drop_graph(c);
+        return plan_linear(c);
+    }
+    if (!strcmp(key, "lin_minb")) {    // register budget / residency of the linear kernel: 4, 5 or 6 CTAs per SM
+        if (value != 4 && value != 5 && value != 6) return fail(BTE_EINVAL, "lin_minb must be 4, 5 or 6");
+        c->lin_minb = (int)value;
+        drop_graph(c);
+        return plan_linear(c);
+    }
+    if (!strcmp(key, "prefetch_rows")) {
         if (value != 0) return fail(BTE_EINVAL, "%s: only 0 (automatic) is supported in this build", key);
         return BTE_OK;
     }

@@ -38,8 +38,11 @@ __device__ __forceinline__ double warp_sum(double v) {
 // Fold of the per-strip partial sums and the per-step bookkeeping of one system, executed by warp 0 of
 // the last block of that system to finish (fixed summation order => deterministic).
 // eq. (12), (20) by the rectangle rule (C10); running sums of eq. (17) for steps k+1 > avg_start (C9).
+//   mode 0: observables only (after init / set_state)
+//   mode 1: observables + running sums + step counter k <- k+1
+//   mode 2: observables + running sums; the step counter is advanced by the caller
 __device__ __forceinline__ void fold_and_advance(const Layout& L, int sys, int n_partials, long long k,
-                                                 bool advance) {
+                                                 int mode) {
     const int lane = threadIdx.x & 31;
     const volatile double* part = L.partial + (size_t)sys * L.pitch * 2;
     double sa = 0.0, sb = 0.0;
@@ -57,7 +60,7 @@ __device__ __forceinline__ void fold_and_advance(const Layout& L, int sys, int n
         st->norm = norm;
         st->v_dr = v;
         st->edge_leak = ((volatile double*)st->edge)[0] + ((volatile double*)st->edge)[1];
-        if (advance) {
+        if (mode != 0) {
             const long long k1 = k + 1;
             if (k1 > c.avg_start_step) {
                 const double t = (double)k1 * L.dt;
@@ -68,7 +71,7 @@ __device__ __forceinline__ void fold_and_advance(const Layout& L, int sys, int n
                 st->sum_s += v * sn * L.dt;
                 st->window += L.dt;
             }
-            st->k = k1;
+            if (mode == 1) st->k = k1;
         }
         st->done = 0u;
         __threadfence();
@@ -87,7 +90,7 @@ __global__ void init_state_kernel(Layout L) {
     }
     if (m >= L.pitch) return;
     double2 w = make_double2(0.0, 0.0);
-    if (m < L.M1) w.x = L.cn[(size_t)sys * (L.N + 1) + n] * L.gm[(size_t)sys * L.pitch + m];
+    if (m < L.M1) w.x = cn_ptr(L, sys)[n] * L.gm[(size_t)sys * L.pitch + m];
     double2* H = state_ptr(L, 0, 0, sys);
     H[(size_t)n * L.pitch + m] = w;
 }
@@ -127,7 +130,7 @@ __global__ void __launch_bounds__(128) half_update_kernel(Layout L, int mode) {
     const double ph = L.phi[(size_t)sys * L.pitch + m];
     const double hba = __dmul_rn(__fma_rn(c.B, ph, Es[0]), 0.5 * delta);
     const double hbb = __dmul_rn(__fma_rn(c.B, ph, Es[1]), 0.5 * delta);
-    const double src = __dmul_rn(L.cn[(size_t)sys * (L.N + 1) + n], __dmul_rn(L.gm[(size_t)sys * L.pitch + m], delta));
+    const double src = __dmul_rn(cn_ptr(L, sys)[n], __dmul_rn(L.gm[(size_t)sys * L.pitch + m], delta));
     const double2 zero = make_double2(0.0, 0.0);
     const bool left = m > 0, right = m + 1 < L.M1;
     const size_t p = (size_t)L.pitch;
@@ -176,7 +179,7 @@ __global__ void __launch_bounds__(256) reduce_finalize_kernel(Layout L, int adva
     }
     __threadfence();
     __syncthreads();
-    if (warp == 0) fold_and_advance(L, sys, blockDim.x >> 5, k, advance != 0);
+    if (warp == 0) fold_and_advance(L, sys, blockDim.x >> 5, k, advance ? 1 : 0);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -261,7 +264,7 @@ __global__ void __launch_bounds__(T) fused_step_kernel(Layout L, int rows_per_ch
 
     const double ph = col_valid ? L.phi[(size_t)sys * L.pitch + col] : 0.0;
     const double gdt = col_valid ? __dmul_rn(L.gm[(size_t)sys * L.pitch + col], L.dt) : 0.0;
-    const double* __restrict__ cn = L.cn + (size_t)sys * (L.N + 1);
+    const double* __restrict__ cn = cn_ptr(L, sys);
     const double kappa = c.kappa_dt;
     const double nu = 1.0 + 0.5 * L.dt, xi = 1.0 - 0.5 * L.dt, nu2 = nu * nu;
     __syncthreads();   // Es visible
@@ -359,7 +362,7 @@ __global__ void __launch_bounds__(T) fused_step_kernel(Layout L, int rows_per_ch
     __syncthreads();
     if (s_last && i < 32) {
         __threadfence();
-        fold_and_advance(L, sys, (int)gridDim.x, k, true);
+        fold_and_advance(L, sys, (int)gridDim.x, k, 1);
     }
 }
 

@@ -14,10 +14,11 @@ from parity_util import assert_obs_close, assert_state_close, oracle_run
 
 pytestmark = pytest.mark.gpu
 
-VARIANTS = {"split": 1, "fused": 2}
+VARIANTS = {"split": 1, "fused": 2, "linear": 3}
+ALL = ["split", "fused", "linear"]
 
 
-def gpu_solver(w, variant="fused", graph_steps=None, tile_rows=None):
+def gpu_solver(w, variant="linear", graph_steps=None, tile_rows=None, ctas=None, minb=None):
     from paper_1401_6047_b200 import Solver
     s = Solver(w.grid, w.params)
     s.set_option("variant", VARIANTS[variant])
@@ -25,12 +26,17 @@ def gpu_solver(w, variant="fused", graph_steps=None, tile_rows=None):
         s.set_option("graph_steps", graph_steps)
     if tile_rows is not None:
         s.set_option("tile_rows", tile_rows)
+    if ctas is not None:
+        s.set_option("tile_cols", ctas)      # number of persistent CTAs of the linear kernel
+    if minb is not None:
+        s.set_option("lin_minb", minb)
     s.init_equilibrium()
     return s
 
 
-def check(w, n_steps, variant, systems=None, graph_steps=None, tile_rows=None, chunks=None):
-    s = gpu_solver(w, variant, graph_steps, tile_rows)
+def check(w, n_steps, variant, systems=None, graph_steps=None, tile_rows=None, chunks=None, ctas=None,
+          minb=None):
+    s = gpu_solver(w, variant, graph_steps, tile_rows, ctas, minb)
     if chunks:                      # several bte_step calls must equal one
         for c in chunks:
             s.step(c)
@@ -51,13 +57,13 @@ def check(w, n_steps, variant, systems=None, graph_steps=None, tile_rows=None, c
 # -------------------------------------------------------------------------------------------------
 # small / ragged shapes
 # -------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("variant", ["split", "fused"])
+@pytest.mark.parametrize("variant", ALL)
 def test_init_equilibrium_matches_oracle(variant):
     w = W.small_case(N=7, M1=45, n_steps=0)
     check(w, 0, variant)
 
 
-@pytest.mark.parametrize("variant", ["split", "fused"])
+@pytest.mark.parametrize("variant", ALL)
 @pytest.mark.parametrize("N,M1", [(1, 3), (2, 5), (5, 126), (12, 127), (9, 128), (33, 253), (40, 801)])
 def test_small_shapes(variant, N, M1):
     """M+1 around the strip width (126 columns) and its multiples, N around the chunk length."""
@@ -72,7 +78,31 @@ def test_fused_row_chunking(tile_rows):
     check(w, 17, "fused", tile_rows=tile_rows)
 
 
-@pytest.mark.parametrize("variant", ["split", "fused"])
+@pytest.mark.parametrize("ctas", [1, 2, 3, 5, 7, 16, 40, 0])
+@pytest.mark.parametrize("minb", [4, 5, 6])
+def test_linear_partition(ctas, minb):
+    """Linearised static partition: CTA ranges that cut strips at arbitrary rows (segments that start at
+    row 0, 1, 2, ..., one-row segments, ranges spanning several strips), all three register budgets."""
+    w = W.small_case(N=21, M1=300, dt=0.004, n_steps=17, avg_start=3)
+    check(w, 17, "linear", ctas=ctas, minb=minb)
+
+
+@pytest.mark.parametrize("ctas", [1, 3, 9, 0])
+def test_linear_partition_batched(ctas):
+    """Ranges spanning several systems, with systems freezing at different steps (on-the-fly compaction)."""
+    w = W.random_batch(n_batch=7, N=9, M1=140, dt=0.004, seed=77, periods=0.2)
+    n = w.n_steps + 3
+    s = gpu_solver(w, "linear", ctas=ctas)
+    s.step(n)
+    obs = s.observables()
+    sims = oracle_run(w, n)
+    for i, sim in sims.items():
+        assert obs[i].step == w.params[i].n_steps_total
+        assert_state_close(s, sim, i, what=f"linbatch[{i}] ctas={ctas}")
+        assert_obs_close(obs[i], sim.observables(), w.params[i], w.grid.dt, what=f"linbatch[{i}] ctas={ctas}")
+
+
+@pytest.mark.parametrize("variant", ALL)
 def test_graph_replay_equals_plain_launches(variant):
     w = W.small_case(N=10, M1=140, n_steps=50, avg_start=7)
     check(w, 50, variant, graph_steps=8)             # 6 graph replays + 2 plain steps
@@ -85,14 +115,15 @@ def test_fused_equals_split_bitwise_state():
     differ only in nothing -- same operation order -- so we ask for exact equality)."""
     w = W.small_case(N=14, M1=260, n_steps=31)
     a = gpu_solver(w, "split"); a.step(31)
-    b = gpu_solver(w, "fused"); b.step(31)
-    for g in (0, 1):
-        xa, xb = a.get_state(0, g)
-        ya, yb = b.get_state(0, g)
-        assert np.array_equal(xa, ya) and np.array_equal(xb, yb)
+    for other in ("fused", "linear"):
+        b = gpu_solver(w, other); b.step(31)
+        for g in (0, 1):
+            xa, xb = a.get_state(0, g)
+            ya, yb = b.get_state(0, g)
+            assert np.array_equal(xa, ya) and np.array_equal(xb, yb), other
 
 
-@pytest.mark.parametrize("variant", ["split", "fused"])
+@pytest.mark.parametrize("variant", ALL)
 def test_batched_with_step_budgets(variant):
     """Config-3-shaped batch: per-system parameters, phi_y ranges and step budgets (systems freeze)."""
     w = W.random_batch(n_batch=6, N=10, M1=150, dt=0.004, seed=123, periods=0.25)
@@ -109,14 +140,14 @@ def test_batched_with_step_budgets(variant):
 
 def test_alpha_and_kappa_scale():
     w = W.small_case(N=8, M1=90, alpha=0.9496, kappa_scale=0.9496, n_steps=20)
-    check(w, 20, "fused")
-    check(w, 20, "split")
+    for v in ALL:
+        check(w, 20, v)
 
 
 def test_set_state_roundtrip_and_step():
     rng = np.random.default_rng(5)
     w = W.small_case(N=6, M1=70, n_steps=9)
-    s = gpu_solver(w, "fused")
+    s = gpu_solver(w, "linear")
     shape = (7, 70)
     ha, hb, fa, fb = (rng.standard_normal(shape) for _ in range(4))
     hb[0] = 0; fb[0] = 0
@@ -148,7 +179,7 @@ def test_create_rejects_unstable_and_invalid():
 # -------------------------------------------------------------------------------------------------
 # BASELINE configs
 # -------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("variant", ["split", "fused"])
+@pytest.mark.parametrize("variant", ALL)
 def test_config0_full(variant):
     from scipy import special
     w = W.config0()
@@ -166,21 +197,21 @@ def test_config1_prefix_and_full_observables():
     """Prefix of 3000 steps: full state parity.  Full length (62 832 steps): observables against the
     oracle values stored in tests/golden/config1_full.json (written by tests/golden/make_golden.py)."""
     w = W.config1()
-    check(w, 3000, "fused")
+    check(w, 3000, "linear")
 
 
 def test_config2_prefix():
     w = W.config2()
-    check(w, 300, "fused")
+    check(w, 300, "linear")
 
 
 def test_config3_subset_prefix():
     """All 512 systems advance together on the GPU; 8 of them (0, 73, 146, ...) are checked."""
     w = W.config3()
-    check(w, 200, "fused", systems=list(range(0, 512, 73)))
+    check(w, 200, "linear", systems=list(range(0, 512, 73)))
 
 
 def test_config4_prefix():
     """Bandwidth-stress grid in the launch configuration bench.py times; 4 steps, full state compare."""
     w = W.config4()
-    check(w, 4, "fused")
+    check(w, 4, "linear")
