@@ -211,6 +211,10 @@ def run_ours(args):
         s.set_option("variant", args.variant)
     if args.tile_rows:
         s.set_option("tile_rows", args.tile_rows)
+    if args.sweep_steps:
+        s.set_option("sweep_steps", args.sweep_steps)
+    if args.ctas:
+        s.set_option("sweep_ctas", args.ctas)
     s.init_equilibrium()
     s.step(max(3, args.warmup))
     barrier()
@@ -249,6 +253,10 @@ def run_ours(args):
         s2.set_option("variant", args.variant)
     if args.tile_rows:
         s2.set_option("tile_rows", args.tile_rows)
+    if args.sweep_steps:
+        s2.set_option("sweep_steps", args.sweep_steps)
+    if args.ctas:
+        s2.set_option("sweep_ctas", args.ctas)
     s2.init_equilibrium()
     s2.step(args.steps)
     obs2 = s2.observables()
@@ -307,6 +315,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 split, 2 fused")
     ap.add_argument("--tile-rows", type=int, default=0)
+    ap.add_argument("--sweep-steps", type=int, default=0, help="steps fused per launch (0 auto)")
+    ap.add_argument("--ctas", type=int, default=0, help="persistent CTAs of the sweep kernel (0 auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -1,12 +1,13 @@
 // bte.cu -- host side of libbte_b200: the C ABI of include/bte.h.
 // Product code: must not include, link or call anything under oracle/.
 #include "../../include/bte.h"
-#include "bte_fused_linear.cuh"
+#include "bte_sweep.cuh"
 
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <algorithm>
 #include <string>
 #include <vector>
 
@@ -59,7 +60,7 @@ Offsets offsets_for(const bte_grid* g) {
     o.phi = off;     off = align_up(off + nb * pitch * sizeof(double));
     o.sc = off;      off = align_up(off + nb * sizeof(SysConst));
     o.ss = off;      off = align_up(off + nb * sizeof(SysState));
-    o.partial = off; off = align_up(off + nb * pitch * 2 * sizeof(double));
+    o.partial = off; off = align_up(off + (size_t)SWEEP_MAX_STEPS * nb * pitch * 2 * sizeof(double));
     o.gctl = off;    off = align_up(off + 64);
     o.total = off;
     return o;
@@ -82,7 +83,7 @@ void bessel_i_ratios(double x, int N, std::vector<double>& r) {
     for (int n = 0; n <= N; ++n) r[n] = t[n] / t[0];
 }
 
-enum Variant { VAR_AUTO = 0, VAR_SPLIT = 1, VAR_FUSED = 2, VAR_LINEAR = 3 };
+enum Variant { VAR_AUTO = 0, VAR_SPLIT = 1, VAR_FUSED = 2, VAR_SWEEP = 3 };
 
 }  // namespace
 
@@ -102,16 +103,18 @@ struct bte_ctx {
     // fused (tile grid) launch plan
     int rows_per_chunk;
     dim3 fgrid;
-    // fused linear (persistent, one wave) launch plan
+    // sweep kernel (persistent, one wave, S steps per launch) launch plan
     bool has_budgets;
-    int lin_grid;        // 0 = variant not usable for this problem
-    int lin_occ, sm_count;
-    int lin_minb;        // __launch_bounds__ min-blocks instantiation of the linear kernel (4, 5 or 6)
+    int sweep_steps;                 // option: 0 = automatic, 1..SWEEP_MAX_STEPS
+    int sweep_ctas;                  // option: grid-size override (0 = SMs x resident CTAs)
+    int sw_grid[SWEEP_MAX_STEPS + 1];   // grid of the S-step kernel; 0 = not usable for this problem
+    int sm_count;
+    std::vector<int64_t> budgets;    // sorted distinct step budgets (n_steps_total > 0)
     // CUDA graph cache
     cudaGraph_t graph;
     cudaGraphExec_t graph_exec;
     int64_t graph_len;
-    int graph_variant;
+    int graph_variant, graph_S;
 };
 
 namespace {
@@ -145,48 +148,76 @@ int plan_fused(bte_ctx* c) {
     return BTE_OK;
 }
 
-using LCfg = LinCfg<FT>;
+// ---- sweep kernel: S leap-frog steps per launch (bte_sweep.cuh) ----------------------------------------
+// resident CTAs per SM the register budget of each instantiation is compiled for
+template <int S> struct SweepMinB { static constexpr int v = S == 1 ? 4 : S == 2 ? 3 : 2; };
 
-void* linear_fn(const bte_ctx* c) {
-    if (c->lin_minb == 4)
-        return c->has_budgets ? (void*)fused_linear_kernel<FT, true, 4> : (void*)fused_linear_kernel<FT, false, 4>;
-    if (c->lin_minb == 6)
-        return c->has_budgets ? (void*)fused_linear_kernel<FT, true, 6> : (void*)fused_linear_kernel<FT, false, 6>;
-    return c->has_budgets ? (void*)fused_linear_kernel<FT, true, 5> : (void*)fused_linear_kernel<FT, false, 5>;
+struct SweepFn { void* fn; size_t smem; int W; };
+
+template <int S>
+SweepFn sweep_fn_s(bool budgets) {
+    using Cfg = SweepCfg<FT, S>;
+    constexpr int MB = SweepMinB<S>::v;
+    return {budgets ? (void*)sweep_kernel<FT, S, true, MB> : (void*)sweep_kernel<FT, S, false, MB>,
+            Cfg::smem_bytes, Cfg::W};
 }
 
-int plan_linear(bte_ctx* c) {
-    c->lin_grid = 0;
-    int dev = 0, sms = 0, occ = 0;
+SweepFn sweep_fn(int S, bool budgets) {
+    switch (S) {
+        case 1: return sweep_fn_s<1>(budgets);
+        case 2: return sweep_fn_s<2>(budgets);
+        case 3: return sweep_fn_s<3>(budgets);
+        default: return sweep_fn_s<4>(budgets);
+    }
+}
+static_assert(SWEEP_MAX_STEPS == 4, "instantiate sweep_kernel for every S up to SWEEP_MAX_STEPS");
+
+int plan_sweep(bte_ctx* c) {
+    int dev = 0, sms = 0;
     CUDA_TRY(cudaGetDevice(&dev));
     CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    void* fn = linear_fn(c);
-    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LCfg::smem_bytes);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, FT, LCfg::smem_bytes);
-    if (e != cudaSuccess) return fail(BTE_ECUDA, "fused_linear_kernel setup failed: %s", cudaGetErrorString(e));
-    if (occ < 1) return BTE_OK;
-    c->lin_occ = occ; c->sm_count = sms;
-    const long long strips = (c->grid.n_phiy + LCfg::W - 1) / LCfg::W;
+    c->sm_count = sms;
     const long long rows_alloc = c->grid.n_harm + 1 + 2 * GHOST;
-    const long long units = strips * (c->grid.n_harm + 1) * (long long)c->grid.n_batch;
-    // 32-bit element offsets inside the kernel: both grids of one buffer, all systems
-    if (2LL * c->grid.n_batch * rows_alloc * c->off.pitch >= (1LL << 31)) return BTE_OK;
-    if (units >= (1LL << 31)) return BTE_OK;
-    long long g = (long long)sms * occ;
-    const long long min_rows = c->tile_cols > 0 ? 1 : 8;   // a CTA should own at least a few rows
-    if (c->tile_cols > 0) g = c->tile_cols;             // option "tile_cols" doubles as a grid-size override
-    if (g > (units + min_rows - 1) / min_rows) g = (units + min_rows - 1) / min_rows;
-    if (g < 1) g = 1;
-    // one CTA range may touch at most MAX_SPAN systems (shared-memory list)
-    if (c->has_budgets && (long long)c->grid.n_batch / g + 2 > LCfg::MAX_SPAN) return BTE_OK;
-    c->lin_grid = (int)g;
+    for (int S = 1; S <= SWEEP_MAX_STEPS; ++S) {
+        c->sw_grid[S] = 0;
+        const SweepFn f = sweep_fn(S, c->has_budgets);
+        int occ = 0;
+        cudaError_t e = cudaFuncSetAttribute(f.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f.smem);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f.fn, FT, f.smem);
+        if (e != cudaSuccess)
+            return fail(BTE_ECUDA, "sweep_kernel<S=%d> setup failed: %s (is this an sm_100a device?)", S,
+                        cudaGetErrorString(e));
+        if (occ < 1) continue;
+        const long long strips = (c->grid.n_phiy + f.W - 1) / f.W;
+        const long long units = strips * (c->grid.n_harm + 1) * (long long)c->grid.n_batch;
+        // 32-bit element offsets inside the kernel: both grids of one buffer, all systems
+        if (2LL * c->grid.n_batch * rows_alloc * c->off.pitch >= (1LL << 31)) continue;
+        if (units >= (1LL << 31)) continue;
+        long long g = (long long)sms * occ;
+        // a CTA should own enough rows to amortise the 3 NS - 1 fill/drain iterations of a segment
+        const long long min_rows = c->sweep_ctas > 0 ? 1 : 8 * S;
+        if (c->sweep_ctas > 0) g = c->sweep_ctas;
+        if (g > (units + min_rows - 1) / min_rows) g = (units + min_rows - 1) / min_rows;
+        if (g < 1) g = 1;
+        // one CTA range may touch at most MAX_SPAN systems (shared-memory list)
+        if (c->has_budgets && (long long)c->grid.n_batch / g + 2 > SweepCfg<FT, 1>::MAX_SPAN) continue;
+        c->sw_grid[S] = (int)g;
+    }
     return BTE_OK;
 }
 
 int effective_variant(const bte_ctx* c) {
-    if (c->variant == VAR_AUTO) return c->lin_grid > 0 ? VAR_LINEAR : VAR_FUSED;
-    if (c->variant == VAR_LINEAR && c->lin_grid == 0) return VAR_FUSED;
+    if (c->variant == VAR_AUTO) return c->sw_grid[1] > 0 ? VAR_SWEEP : VAR_FUSED;
+    if (c->variant == VAR_SWEEP && c->sw_grid[1] == 0) return VAR_FUSED;
     return c->variant;
+}
+
+// steps fused per launch by the sweep kernel (the other variants advance one step per launch group)
+int sweep_steps(const bte_ctx* c) {
+    if (effective_variant(c) != VAR_SWEEP) return 1;
+    int S = c->sweep_steps > 0 ? c->sweep_steps : 2;
+    while (S > 1 && c->sw_grid[S] == 0) --S;
+    return S;
 }
 
 void drop_graph(bte_ctx* c) {
@@ -204,12 +235,13 @@ dim3 split_grid(const bte_ctx* c) {
 
 int launches_per_step(const bte_ctx* c) { return effective_variant(c) == VAR_SPLIT ? 3 : 1; }
 
-// Issue one step with plain launches.
-int launch_step(bte_ctx* c) {
+// Issue one launch group with plain launches: S steps (sweep kernel) or one step (other variants).
+int launch_steps(bte_ctx* c, int S) {
     const int var = effective_variant(c);
-    if (var == VAR_LINEAR) {
+    if (var == VAR_SWEEP) {
+        const SweepFn f = sweep_fn(S, c->has_budgets);
         void* args[] = {&c->L};
-        CUDA_TRY(cudaLaunchKernel(linear_fn(c), dim3(c->lin_grid), dim3(FT), args, LCfg::smem_bytes, c->stream));
+        CUDA_TRY(cudaLaunchKernel(f.fn, dim3(c->sw_grid[S]), dim3(FT), args, f.smem, c->stream));
     } else if (var == VAR_FUSED) {
         fused_step_kernel<FT, FD><<<c->fgrid, FT, FCfg::smem_bytes, c->stream>>>(c->L, c->rows_per_chunk);
     } else {
@@ -223,10 +255,10 @@ int launch_step(bte_ctx* c) {
     return BTE_OK;
 }
 
-// Build a graph of `len` steps from explicit kernel nodes (no stream capture: safe with any caller
-// stream).  Kernels take no per-step argument -- the step counter lives on the device -- so one graph
-// can be replayed any number of times.
-int build_graph(bte_ctx* c, int64_t len) {
+// Build a graph of `len` launch groups (each S steps) from explicit kernel nodes (no stream capture: safe
+// with any caller stream).  Kernels take no per-step argument -- the step counter lives on the device -- so
+// one graph can be replayed any number of times.
+int build_graph(bte_ctx* c, int64_t len, int S) {
     drop_graph(c);
     CUDA_TRY(cudaGraphCreate(&c->graph, 0));
     cudaGraphNode_t prev = nullptr;
@@ -243,9 +275,10 @@ int build_graph(bte_ctx* c, int64_t len) {
             prev = node;
             return e;
         };
-        if (var == VAR_LINEAR) {
+        if (var == VAR_SWEEP) {
+            const SweepFn f = sweep_fn(S, c->has_budgets);
             void* args[] = {&c->L};
-            CUDA_TRY(add(linear_fn(c), dim3(c->lin_grid), dim3(FT), LCfg::smem_bytes, args));
+            CUDA_TRY(add(f.fn, dim3(c->sw_grid[S]), dim3(FT), f.smem, args));
         } else if (var == VAR_FUSED) {
             void* args[] = {&c->L, &rpc};
             CUDA_TRY(add((void*)fused_step_kernel<FT, FD>, c->fgrid, dim3(FT), FCfg::smem_bytes, args));
@@ -262,6 +295,7 @@ int build_graph(bte_ctx* c, int64_t len) {
     CUDA_TRY(cudaGraphInstantiate(&c->graph_exec, c->graph, 0));
     c->graph_len = len;
     c->graph_variant = var;
+    c->graph_S = S;
     return BTE_OK;
 }
 
@@ -272,9 +306,20 @@ int64_t auto_graph_steps(const bte_ctx* c) {
     return 64;
 }
 
-int64_t system_steps(const bte_ctx* c, int sys) {
-    const int64_t tot = c->params[sys].n_steps_total;
-    return (tot > 0 && c->steps_issued > tot) ? tot : c->steps_issued;
+// steps until the next step budget strictly after global step k (INT64_MAX if none)
+int64_t steps_to_next_budget(const bte_ctx* c, int64_t k) {
+    auto it = std::upper_bound(c->budgets.begin(), c->budgets.end(), k);
+    return it == c->budgets.end() ? INT64_MAX : *it - k;
+}
+
+// which ping-pong buffer holds the current state of a system (device-side flag; synchronises the stream)
+int live_buffer(bte_ctx* c, int sys, int* buf) {
+    SysState st;
+    CUDA_TRY(cudaMemcpyAsync(&st, c->ws + c->off.ss + (size_t)sys * sizeof(SysState), sizeof(SysState),
+                             cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    *buf = st.buf & 1;
+    return BTE_OK;
 }
 
 }  // namespace
@@ -349,7 +394,7 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
     CUDA_TRY(cudaMemcpyAsync(ws + off.sc, sc.data(), sc.size() * sizeof(SysConst), cudaMemcpyHostToDevice, stream));
     CUDA_TRY(cudaMemsetAsync(ws + off.state, 0, off.state_bytes, stream));   // ghost rows stay zero forever
     CUDA_TRY(cudaMemsetAsync(ws + off.ss, 0, (size_t)nb * sizeof(SysState), stream));
-    CUDA_TRY(cudaMemsetAsync(ws + off.partial, 0, (size_t)nb * pitch * 2 * sizeof(double), stream));
+    CUDA_TRY(cudaMemsetAsync(ws + off.partial, 0, (size_t)SWEEP_MAX_STEPS * nb * pitch * 2 * sizeof(double), stream));
     CUDA_TRY(cudaMemsetAsync(ws + off.gctl, 0, 64, stream));
     CUDA_TRY(cudaStreamSynchronize(stream));   // host tables go out of scope
 
@@ -370,7 +415,12 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
     c->L.gctl = (unsigned int*)(ws + off.gctl);
     c->has_budgets = false;
     for (int s = 0; s < nb; ++s) c->has_budgets = c->has_budgets || params[s].n_steps_total > 0;
-    c->lin_grid = 0; c->lin_occ = 0; c->sm_count = 0; c->lin_minb = 4;
+    for (int s = 0; s < nb; ++s)
+        if (params[s].n_steps_total > 0) c->budgets.push_back(params[s].n_steps_total);
+    std::sort(c->budgets.begin(), c->budgets.end());
+    c->budgets.erase(std::unique(c->budgets.begin(), c->budgets.end()), c->budgets.end());
+    c->sweep_steps = 0; c->sweep_ctas = 0; c->sm_count = 0; c->graph_S = 0;
+    for (int S = 0; S <= SWEEP_MAX_STEPS; ++S) c->sw_grid[S] = 0;
     c->steps_issued = 0; c->launches = 0;
     c->variant = VAR_AUTO; c->graph_steps = -1;
     c->tile_cols = 0; c->tile_rows = 0; c->prefetch_rows = 0;
@@ -383,7 +433,7 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
         delete c;
         return fail(BTE_ECUDA, "cudaFuncSetAttribute failed: %s (is this an sm_100a device?)", cudaGetErrorString(e));
     }
-    rc = plan_linear(c);
+    rc = plan_sweep(c);
     if (rc != BTE_OK) { delete c; return rc; }
     *out = c;
     return BTE_OK;
@@ -405,23 +455,33 @@ int bte_step(bte_ctx* c, int64_t n_steps) {
     if (!c) return fail(BTE_EINVAL, "bte_step: NULL ctx");
     if (n_steps < 0) return fail(BTE_EINVAL, "bte_step: n_steps < 0");
     int64_t left = n_steps;
-    const int64_t glen = c->graph_steps < 0 ? auto_graph_steps(c) : c->graph_steps;
-    if (glen > 1 && left >= glen) {
-        if (!c->graph_exec || c->graph_len != glen || c->graph_variant != effective_variant(c)) {
-            int rc = build_graph(c, glen);
+    const int S = sweep_steps(c);
+    const int var = effective_variant(c);
+    // launch-bound grids: replay a graph of glen launch groups of S steps each (not with step budgets:
+    // a budget boundary inside a group changes the group)
+    const int64_t glen = c->has_budgets ? 0 : (c->graph_steps < 0 ? auto_graph_steps(c) : c->graph_steps);
+    if (glen > 1 && left >= glen * S) {
+        if (!c->graph_exec || c->graph_len != glen || c->graph_variant != var || c->graph_S != S) {
+            int rc = build_graph(c, glen, S);
             if (rc != BTE_OK) return rc;
         }
-        while (left >= glen) {
+        while (left >= glen * S) {
             CUDA_TRY(cudaGraphLaunch(c->graph_exec, c->stream));
             c->launches += glen * launches_per_step(c);
-            left -= glen;
+            left -= glen * S;
+            c->steps_issued += glen * S;
         }
     }
-    for (; left > 0; --left) {
-        int rc = launch_step(c);
+    while (left > 0) {
+        // an s-step launch must not contain a budget boundary in its interior (a system that would freeze
+        // after fewer than s steps): shorten the group to end exactly on the next boundary
+        int64_t s = std::min<int64_t>(S, left);
+        if (c->has_budgets) s = std::min<int64_t>(s, steps_to_next_budget(c, c->steps_issued));
+        int rc = launch_steps(c, (int)s);
         if (rc != BTE_OK) return rc;
+        left -= s;
+        c->steps_issued += s;
     }
-    c->steps_issued += n_steps;
     return BTE_OK;
 }
 
@@ -451,7 +511,8 @@ int bte_get_state(bte_ctx* c, int32_t system, int32_t grid_id, double* a, double
     if (system < 0 || system >= c->grid.n_batch || grid_id < 0 || grid_id > 1)
         return fail(BTE_EINVAL, "bte_get_state: bad system or grid index");
     const int rows = c->grid.n_harm + 1, M1 = c->grid.n_phiy, pitch = c->off.pitch;
-    const int buf = (int)(system_steps(c, system) & 1);
+    int buf = 0;
+    { const int rc = live_buffer(c, system, &buf); if (rc != BTE_OK) return rc; }
     const size_t gp = (size_t)(rows + 2 * GHOST) * pitch, row0 = (size_t)GHOST * pitch;
     const double2* z = c->L.state + (((size_t)buf * 2 + grid_id) * c->grid.n_batch + system) * gp + row0;
     // rows 0..N of the other buffer of this (grid, system) are dead between steps: use them as staging
@@ -472,7 +533,8 @@ int bte_set_state(bte_ctx* c, int32_t system, int32_t grid_id, const double* a, 
     if (system < 0 || system >= c->grid.n_batch || grid_id < 0 || grid_id > 1)
         return fail(BTE_EINVAL, "bte_set_state: bad system or grid index");
     const int rows = c->grid.n_harm + 1, M1 = c->grid.n_phiy, pitch = c->off.pitch;
-    const int buf = (int)(system_steps(c, system) & 1);
+    int buf = 0;
+    { const int rc = live_buffer(c, system, &buf); if (rc != BTE_OK) return rc; }
     const size_t gp = (size_t)(rows + 2 * GHOST) * pitch, row0 = (size_t)GHOST * pitch;
     double2* z = c->L.state + (((size_t)buf * 2 + grid_id) * c->grid.n_batch + system) * gp + row0;
     double* stage = (double*)(c->L.state + (((size_t)(buf ^ 1) * 2 + grid_id) * c->grid.n_batch + system) * gp + row0);
@@ -483,7 +545,7 @@ int bte_set_state(bte_ctx* c, int32_t system, int32_t grid_id, const double* a, 
     interleave_kernel<<<g, 256, 0, c->stream>>>(z, stage, stage + cnt, rows, M1, pitch);
     c->launches += 1;
     if (grid_id == 0) {   // keep norm / v_dr of the observables consistent with the new whole grid
-        // reduce_finalize reads buffer (k & 1) of every system; harmless for the others
+        // reduce_finalize reads the live buffer of every system; harmless for the others
         reduce_finalize_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 0);
         c->launches += 1;
     }
@@ -511,17 +573,17 @@ int bte_set_option(bte_ctx* c, const char* key, int64_t value) {
         drop_graph(c);
         return plan_fused(c);
     }
-    if (!strcmp(key, "tile_cols")) {   // CTAs of the persistent fused_linear_kernel (0 = SMs x occupancy)
-        if (value < 0 || value > 65535) return fail(BTE_EINVAL, "tile_cols must be in [0, 65535]");
-        c->tile_cols = (int)value;
+    if (!strcmp(key, "sweep_ctas") || !strcmp(key, "tile_cols")) {   // CTAs of the persistent sweep kernel (0 = SMs x occupancy)
+        if (value < 0 || value > 65535) return fail(BTE_EINVAL, "%s must be in [0, 65535]", key);
+        c->sweep_ctas = (int)value;
         drop_graph(c);
-        return plan_linear(c);
+        return plan_sweep(c);
     }
-    if (!strcmp(key, "lin_minb")) {    // register budget / residency of the linear kernel: 4, 5 or 6 CTAs per SM
-        if (value != 4 && value != 5 && value != 6) return fail(BTE_EINVAL, "lin_minb must be 4, 5 or 6");
-        c->lin_minb = (int)value;
+    if (!strcmp(key, "sweep_steps")) {   // leap-frog steps fused per launch of the sweep kernel (0 = automatic)
+        if (value < 0 || value > SWEEP_MAX_STEPS) return fail(BTE_EINVAL, "sweep_steps must be in [0, %d]", SWEEP_MAX_STEPS);
+        c->sweep_steps = (int)value;
         drop_graph(c);
-        return plan_linear(c);
+        return BTE_OK;
     }
     if (!strcmp(key, "prefetch_rows")) {
         if (value != 0) return fail(BTE_EINVAL, "%s: only 0 (automatic) is supported in this build", key);

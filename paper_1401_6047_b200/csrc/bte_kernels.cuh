@@ -39,7 +39,7 @@ __device__ __forceinline__ double warp_sum(double v) {
 // the last block of that system to finish (fixed summation order => deterministic).
 // eq. (12), (20) by the rectangle rule (C10); running sums of eq. (17) for steps k+1 > avg_start (C9).
 //   mode 0: observables only (after init / set_state)
-//   mode 1: observables + running sums + step counter k <- k+1
+//   mode 1: observables + running sums + step counter k <- k+1, live buffer toggled
 //   mode 2: observables + running sums; the step counter is advanced by the caller
 __device__ __forceinline__ void fold_and_advance(const Layout& L, int sys, int n_partials, long long k,
                                                  int mode) {
@@ -71,7 +71,7 @@ __device__ __forceinline__ void fold_and_advance(const Layout& L, int sys, int n
                 st->sum_s += v * sn * L.dt;
                 st->window += L.dt;
             }
-            if (mode == 1) st->k = k1;
+            if (mode == 1) { st->k = k1; st->buf ^= 1; }
         }
         st->done = 0u;
         __threadfence();
@@ -107,7 +107,7 @@ __global__ void __launch_bounds__(128) half_update_kernel(Layout L, int mode) {
     const SysConst c = L.sc[sys];
     const long long k = (mode == 2) ? 0 : L.ss[sys].k;
     if (mode != 2 && c.n_steps_total > 0 && k >= c.n_steps_total) return;   // frozen system
-    const int cur = (int)(k & 1), nxt = cur ^ 1;
+    const int cur = (mode == 2) ? 0 : L.ss[sys].buf, nxt = cur ^ 1;
     const double2 *X, *S;
     double2* O;
     double delta, ta, tb;
@@ -151,14 +151,14 @@ __global__ void __launch_bounds__(128) half_update_kernel(Layout L, int mode) {
     O[n * p + m] = w;
 }
 
-// One block per system: sums row 0 (a) and row 1 (b) of the whole grid in buffer ((k + advance) & 1),
+// One block per system: sums row 0 (a) and row 1 (b) of the whole grid in buffer (buf ^ advance),
 // then folds.  Used by the split variant (advance = 1) and after init / set_state (advance = 0).
 __global__ void __launch_bounds__(256) reduce_finalize_kernel(Layout L, int advance) {
     const int sys = blockIdx.x;
     const SysConst c = L.sc[sys];
     const long long k = L.ss[sys].k;
     if (advance && c.n_steps_total > 0 && k >= c.n_steps_total) return;
-    const int buf = (int)((k + (advance ? 1 : 0)) & 1);
+    const int buf = L.ss[sys].buf ^ (advance ? 1 : 0);
     const double2* H = state_ptr(L, buf, 0, sys);
     double sa = 0.0, sb = 0.0;
     for (int m = threadIdx.x; m < L.M1; m += blockDim.x) {
@@ -220,7 +220,7 @@ __global__ void __launch_bounds__(T) fused_step_kernel(Layout L, int rows_per_ch
     const SysConst c = L.sc[sys];
     const long long k = L.ss[sys].k;
     if (c.n_steps_total > 0 && k >= c.n_steps_total) return;   // frozen system: nothing to do
-    const int cur = (int)(k & 1), nxt = cur ^ 1;
+    const int cur = L.ss[sys].buf, nxt = cur ^ 1;
     const double2* __restrict__ Hold = state_ptr(L, cur, 0, sys);
     const double2* __restrict__ Fold = state_ptr(L, cur, 1, sys);
     double2* __restrict__ Hnew = state_ptr(L, nxt, 0, sys);

@@ -14,29 +14,30 @@ from parity_util import assert_obs_close, assert_state_close, oracle_run
 
 pytestmark = pytest.mark.gpu
 
-VARIANTS = {"split": 1, "fused": 2, "linear": 3}
-ALL = ["split", "fused", "linear"]
+# name -> (variant, leap-frog steps fused per launch of the sweep kernel)
+VARIANTS = {"split": (1, 0), "fused": (2, 0), "sweep1": (3, 1), "sweep2": (3, 2), "sweep3": (3, 3),
+            "sweep4": (3, 4), "auto": (0, 0)}
+SWEEPS = ["sweep1", "sweep2", "sweep3", "sweep4"]
+ALL = ["split", "fused"] + SWEEPS
 
 
-def gpu_solver(w, variant="linear", graph_steps=None, tile_rows=None, ctas=None, minb=None):
+def gpu_solver(w, variant="auto", graph_steps=None, tile_rows=None, ctas=None):
     from paper_1401_6047_b200 import Solver
     s = Solver(w.grid, w.params)
-    s.set_option("variant", VARIANTS[variant])
+    s.set_option("variant", VARIANTS[variant][0])
+    s.set_option("sweep_steps", VARIANTS[variant][1])
     if graph_steps is not None:
         s.set_option("graph_steps", graph_steps)
     if tile_rows is not None:
         s.set_option("tile_rows", tile_rows)
     if ctas is not None:
-        s.set_option("tile_cols", ctas)      # number of persistent CTAs of the linear kernel
-    if minb is not None:
-        s.set_option("lin_minb", minb)
+        s.set_option("sweep_ctas", ctas)     # number of persistent CTAs of the sweep kernel
     s.init_equilibrium()
     return s
 
 
-def check(w, n_steps, variant, systems=None, graph_steps=None, tile_rows=None, chunks=None, ctas=None,
-          minb=None):
-    s = gpu_solver(w, variant, graph_steps, tile_rows, ctas, minb)
+def check(w, n_steps, variant, systems=None, graph_steps=None, tile_rows=None, chunks=None, ctas=None):
+    s = gpu_solver(w, variant, graph_steps, tile_rows, ctas)
     if chunks:                      # several bte_step calls must equal one
         for c in chunks:
             s.step(c)
@@ -79,20 +80,22 @@ def test_fused_row_chunking(tile_rows):
 
 
 @pytest.mark.parametrize("ctas", [1, 2, 3, 5, 7, 16, 40, 0])
-@pytest.mark.parametrize("minb", [4, 5, 6])
-def test_linear_partition(ctas, minb):
+@pytest.mark.parametrize("variant", SWEEPS)
+def test_sweep_partition(ctas, variant):
     """Linearised static partition: CTA ranges that cut strips at arbitrary rows (segments that start at
-    row 0, 1, 2, ..., one-row segments, ranges spanning several strips), all three register budgets."""
+    row 0, 1, 2, ..., one-row segments, ranges spanning several strips), every sweep depth S; 17 steps
+    is not a multiple of S = 2, 3, 4, so the trailing shorter launch is covered too."""
     w = W.small_case(N=21, M1=300, dt=0.004, n_steps=17, avg_start=3)
-    check(w, 17, "linear", ctas=ctas, minb=minb)
+    check(w, 17, variant, ctas=ctas)
 
 
 @pytest.mark.parametrize("ctas", [1, 3, 9, 0])
-def test_linear_partition_batched(ctas):
+@pytest.mark.parametrize("variant", SWEEPS)
+def test_sweep_partition_batched(ctas, variant):
     """Ranges spanning several systems, with systems freezing at different steps (on-the-fly compaction)."""
     w = W.random_batch(n_batch=7, N=9, M1=140, dt=0.004, seed=77, periods=0.2)
     n = w.n_steps + 3
-    s = gpu_solver(w, "linear", ctas=ctas)
+    s = gpu_solver(w, variant, ctas=ctas)
     s.step(n)
     obs = s.observables()
     sims = oracle_run(w, n)
@@ -115,7 +118,7 @@ def test_fused_equals_split_bitwise_state():
     differ only in nothing -- same operation order -- so we ask for exact equality)."""
     w = W.small_case(N=14, M1=260, n_steps=31)
     a = gpu_solver(w, "split"); a.step(31)
-    for other in ("fused", "linear"):
+    for other in ["fused"] + SWEEPS:
         b = gpu_solver(w, other); b.step(31)
         for g in (0, 1):
             xa, xb = a.get_state(0, g)
@@ -147,7 +150,7 @@ def test_alpha_and_kappa_scale():
 def test_set_state_roundtrip_and_step():
     rng = np.random.default_rng(5)
     w = W.small_case(N=6, M1=70, n_steps=9)
-    s = gpu_solver(w, "linear")
+    s = gpu_solver(w, "auto")
     shape = (7, 70)
     ha, hb, fa, fb = (rng.standard_normal(shape) for _ in range(4))
     hb[0] = 0; fb[0] = 0
@@ -197,21 +200,21 @@ def test_config1_prefix_and_full_observables():
     """Prefix of 3000 steps: full state parity.  Full length (62 832 steps): observables against the
     oracle values stored in tests/golden/config1_full.json (written by tests/golden/make_golden.py)."""
     w = W.config1()
-    check(w, 3000, "linear")
+    check(w, 3000, "auto")
 
 
 def test_config2_prefix():
     w = W.config2()
-    check(w, 300, "linear")
+    check(w, 300, "auto")
 
 
 def test_config3_subset_prefix():
     """All 512 systems advance together on the GPU; 8 of them (0, 73, 146, ...) are checked."""
     w = W.config3()
-    check(w, 200, "linear", systems=list(range(0, 512, 73)))
+    check(w, 200, "auto", systems=list(range(0, 512, 73)))
 
 
 def test_config4_prefix():
     """Bandwidth-stress grid in the launch configuration bench.py times; 4 steps, full state compare."""
     w = W.config4()
-    check(w, 4, "linear")
+    check(w, 4, "auto")
