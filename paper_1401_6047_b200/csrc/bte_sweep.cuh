@@ -42,10 +42,10 @@ struct SweepCfg {
     static constexpr int QD = 8;               // depth of a stage ring that is read back as "own" (4 iterations later)
     static constexpr int ring_rows = (NS - 2) * QD + 2;   // stages 0..NS-3: QD slots; stage NS-2: 2 slots
     static constexpr int MAX_SPAN = 64;        // distinct systems one CTA range may touch
-    static constexpr int CS = 16;              // slots of the c_n ring
-    static constexpr size_t smem_bytes = sizeof(double2) * ((size_t)R * (FCOLS + T) + (size_t)ring_rows * SC);
+    static constexpr int CS = 32;              // slots of the c_n ring (unit v brings c of its row into slot v & 31)
+    static constexpr size_t smem_bytes = sizeof(double2) * ((size_t)R * (FCOLS + T) + (size_t)ring_rows * SC) + CS * sizeof(double);
     static_assert(W >= 32, "strip too narrow");
-    static_assert(2 * (NS - 1) + 2 <= CS, "c_n ring too short");
+    static_assert(2 * (NS - 1) + 1 + D + 2 <= CS, "c_n ring too short");
 };
 
 // active for an S-step launch: no budget, or at least S steps left (the host never issues an S-step launch
@@ -65,6 +65,15 @@ __device__ __forceinline__ void cp_async16_sz_if(unsigned smem_addr, const void*
     asm volatile(
         "{\n .reg .pred p;\n setp.ne.s32 p, %3, 0;\n"
         " @p cp.async.cg.shared.global [%0], [%1], 16, %2;\n}\n" ::"r"(smem_addr),
+        "l"(gmem_src), "r"(src_bytes), "r"(pred)
+        : "memory");
+}
+// 8-byte copy issued by thread 0 only (c_n of the row of a load unit); src_bytes 0 => zero fill
+__device__ __forceinline__ void cp_async8_sz_if(unsigned smem_addr, const void* gmem_src, int src_bytes,
+                                                int pred) {
+    asm volatile(
+        "{\n .reg .pred p;\n setp.ne.s32 p, %3, 0;\n"
+        " @p cp.async.ca.shared.global [%0], [%1], 8, %2;\n}\n" ::"r"(smem_addr),
         "l"(gmem_src), "r"(src_bytes), "r"(pred)
         : "memory");
 }
@@ -127,7 +136,6 @@ __device__ __forceinline__ void fold_sweep(const Layout& L, int sys, int n_parti
 template <int T, int S>
 struct SweepShared {
     double Es[2 * S + 2];            // E(t_k + v dt/2), v = 0 .. NS+1  (C14)
-    double cs[SweepCfg<T, S>::CS];   // ring of c_n: slot v & 15 holds c of stage 0's row at iteration v
     double red[T / 32];
     double acc[S][2][T];             // rows 0 (a) and 1 (b) of the S new whole grids, per owned column
     int scan[T / 32];
@@ -147,7 +155,7 @@ __device__ __forceinline__ void sweep_segment(const Layout& L, const int sys, co
     const int i = threadIdx.x;
     const unsigned sF = (unsigned)__cvta_generic_to_shared(smem);          // F^0 ring [R][FCOLS]
     const unsigned sH = sF + R * FROW;                                      // H^0 ring [R][T]
-    const unsigned sC = (unsigned)__cvta_generic_to_shared(sh.cs);
+    const unsigned sC = sH + R * HROW + Cfg::ring_rows * SROW;             // c_n ring [CS] doubles
 
     const SysConst c = L.sc[sys];
     const long long k = L.ss[sys].k;
@@ -171,7 +179,7 @@ __device__ __forceinline__ void sweep_segment(const Layout& L, const int sys, co
     const int ipitch = L.pitch;
     const int adjH = col_valid ? col : 0;
     const int adjF = (szF ? cf : 0) + Y, adjF2 = ((i < 2 && szF2) ? cf2 : 0) + Y;
-    const int two = (i < 2) ? 1 : 0;
+    const int two = (i < 2) ? 1 : 0, first = (i == 0) ? 1 : 0;
 
     __syncthreads();   // the previous segment (or the scan) is done with the rings / sh
     if (i < NS + 2) sh.Es[i] = field_E(c, ((double)k + 0.5 * (double)i) * L.dt);   // (C14)
@@ -185,13 +193,6 @@ __device__ __forceinline__ void sweep_segment(const Layout& L, const int sys, co
     const int n_iter = Lr + 3 * NS - 1;
     const int row_first = r0 - NS - 1;                 // stage 0's row at iteration u is row_first + u
 
-    auto load_cn = [&](int r) { return (r >= -GHOST && r <= L.N + GHOST) ? __ldg(cn0 + r) : 0.0; };
-    double creg = 0.0;                                 // thread 0: c of stage 0's row two iterations ahead
-    if (i == 0) {
-        sh.cs[u_start & (Cfg::CS - 1)] = load_cn(row_first + u_start);
-        creg = load_cn(row_first + u_start + 1);
-    }
-
     // issue of load unit v (F^0 row r0-NS+v, H^0 row r0-NS+v) into ring slot v & 7
     int off_in = (r0 - NS + u_start) * ipitch;         // element offset of the next unit's row
     auto issue_edge = [&](int v) {
@@ -203,6 +204,7 @@ __device__ __forceinline__ void sweep_segment(const Layout& L, const int sys, co
             cp_async16_sz(sF + slot * FROW + i * 16, Hold + (o + adjF), in ? szF : 0);
             cp_async16_sz_if(sF + slot * FROW + (T + i) * 16, Hold + (o + adjF2), in ? szF2 : 0, two);
             if (v >= 1 && v <= Lr + 2 * NS - 2) cp_async16_sz(sH + slot * HROW + i * 16, Hold + (o + adjH), in ? szH : 0);
+            cp_async8_sz_if(sC + (unsigned)(v & (Cfg::CS - 1)) * 8, cn0 + (in ? row : 0), in ? 8 : 0, first);
         }
         cp_async_commit();
         off_in += ipitch;
@@ -245,39 +247,45 @@ __device__ __forceinline__ void sweep_segment(const Layout& L, const int sys, co
 
         cp_async_wait<D>();   // this thread's copies of unit u have landed
         __syncthreads();      // ... everybody's; orders the stage rings; frees slot (u-4) & 7
-        if (i == 0) {         // c_n ring: publish c of stage 0's row of the NEXT iteration, fetch one further
-            sh.cs[(u + 1) & (Cfg::CS - 1)] = creg;
-            creg = load_cn(row0 + 2);
-        }
         if (EDGE) {
             issue_edge(u + D + 1);
         } else {
             cp_async16_sz(tF + si * FROW, Hold + (off_in + adjF), szF);
             cp_async16_sz_if(tF + si * FROW + T * 16, Hold + (off_in + adjF2), szF2, two);
             cp_async16_sz(tF + tH_off + si * HROW, Hold + (off_in + adjH), szH);
+            cp_async8_sz_if(sC + (unsigned)((u + D + 1) & (Cfg::CS - 1)) * 8, cn0 + (row0 + D + 2), 8, first);
             cp_async_commit();
             off_in += ipitch;
         }
+        // phase 1: every shared-memory read of this iteration (all of them target slots written in earlier
+        // iterations, so they are independent of this iteration's results and can be in flight together)
+        double2 d0s[NS], ws[NS];
+        double cjs[NS];
 #pragma unroll
         for (int j = 0; j < NS; ++j) {
             const int row = row0 - 2 * j;                            // row formed by stage j
             // phi_y-difference of row+1 of the stencil grid X^j (row 0 pre-doubled in a: chi(1) = 2, eq. 11)
-            double2 d0;
             {
                 unsigned a;
                 if (j == 0) a = tF + o_u;                                        // F^0, columns col-1 / col+1
                 else if (j == NS - 1) a = tF + tQ_off + (NS - 2) * QD * SROW + l_p;
                 else a = tF + tQ_off + (j - 1) * QD * SROW + q_p;
                 const double2 l = lds_d2(a), r = lds_d2(a + 32);
-                d0.x = __dsub_rn(r.x, l.x); d0.y = __dsub_rn(r.y, l.y);
-                if (EDGE && row + 1 == 0) d0.x *= 2.0;
+                d0s[j].x = __dsub_rn(r.x, l.x); d0s[j].y = __dsub_rn(r.y, l.y);
+                if (EDGE && row + 1 == 0) d0s[j].x *= 2.0;
             }
             // own point: X^{j-1}[row][col]
-            double2 w;
-            if (j == 0) w = lds_d2(tF + tH_off + o_h);
-            else if (j == 1) w = lds_d2(tF + o_f + 16);
-            else w = lds_d2(tF + tQ_off + (j - 2) * QD * SROW + q_o + 16);
-            const double cj = lds_d(sC + (unsigned)((u - 2 * j) & (Cfg::CS - 1)) * 8);
+            if (j == 0) ws[j] = lds_d2(tF + tH_off + o_h);
+            else if (j == 1) ws[j] = lds_d2(tF + o_f + 16);
+            else ws[j] = lds_d2(tF + tQ_off + (j - 2) * QD * SROW + q_o + 16);
+            cjs[j] = lds_d(sC + (unsigned)((u - 1 - 2 * j) & (Cfg::CS - 1)) * 8);   // unit u-1-2j = this row
+        }
+        // phase 2: the NS half-updates
+#pragma unroll
+        for (int j = 0; j < NS; ++j) {
+            const int row = row0 - 2 * j;
+            const double2 d0 = d0s[j], w = ws[j];
+            const double cj = cjs[j];
             double2 out = cn_point(w, d2[j], d0, nd0 - (double)(2 * j), hb[j], hb[j + 2], __dmul_rn(cj, gdt),
                                    kappa, L.xi, L.nu, L.nu2);
             if (EDGE) {
