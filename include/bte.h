@@ -121,7 +121,7 @@ int bte_set_state(bte_ctx* ctx, int32_t system, int32_t grid_id, const double* a
  *   "variant"      0 = automatic (default), 1 = two half-update kernels per step (96 B/point/step),
  *                  2 = fused whole+fractional kernel on a 2-D tile grid (64 B/point/step),
  *                  3 = persistent sweep kernel, S steps per launch (64/S B/point/step; the default path)
- *   "sweep_steps"  S of variant 3: 1..4, 0 = automatic
+ *   "sweep_steps"  S of variant 3: 1..3, 0 = automatic
  *   "sweep_ctas"   CTAs of the persistent sweep kernel, 0 = SMs x resident CTAs
  *   "graph_steps"  launches captured per CUDA graph for launch-bound grids; 0 = plain launches, -1 = auto
  *   "tile_rows"    rows per tile of variant 2 (0 = automatic)

@@ -166,11 +166,10 @@ SweepFn sweep_fn(int S, bool budgets) {
     switch (S) {
         case 1: return sweep_fn_s<1>(budgets);
         case 2: return sweep_fn_s<2>(budgets);
-        case 3: return sweep_fn_s<3>(budgets);
-        default: return sweep_fn_s<4>(budgets);
+        default: return sweep_fn_s<3>(budgets);
     }
 }
-static_assert(SWEEP_MAX_STEPS == 4, "instantiate sweep_kernel for every S up to SWEEP_MAX_STEPS");
+static_assert(SWEEP_MAX_STEPS == 3, "instantiate sweep_kernel for every S up to SWEEP_MAX_STEPS");
 
 int plan_sweep(bte_ctx* c) {
     int dev = 0, sms = 0;
@@ -215,7 +214,9 @@ int effective_variant(const bte_ctx* c) {
 // steps fused per launch by the sweep kernel (the other variants advance one step per launch group)
 int sweep_steps(const bte_ctx* c) {
     if (effective_variant(c) != VAR_SWEEP) return 1;
-    int S = c->sweep_steps > 0 ? c->sweep_steps : 2;
+    // automatic depth: 3 steps per pass when the march over n is long enough to amortise the 3 NS - 1
+    // fill/drain iterations of a segment, else 2 (measured on configs 3 and 4)
+    int S = c->sweep_steps > 0 ? c->sweep_steps : (c->grid.n_harm + 1 >= 96 ? 3 : 2);
     while (S > 1 && c->sw_grid[S] == 0) --S;
     return S;
 }

@@ -42,10 +42,10 @@ struct SweepCfg {
     static constexpr int QD = 8;               // depth of a stage ring that is read back as "own" (4 iterations later)
     static constexpr int ring_rows = (NS - 2) * QD + 2;   // stages 0..NS-3: QD slots; stage NS-2: 2 slots
     static constexpr int MAX_SPAN = 64;        // distinct systems one CTA range may touch
-    static constexpr int CS = 32;              // slots of the c_n ring (unit v brings c of its row into slot v & 31)
+    static constexpr int CS = 32;              // c_n ring: unit v brings c of its row into slots v & 15 and (v & 15) + 16
     static constexpr size_t smem_bytes = sizeof(double2) * ((size_t)R * (FCOLS + T) + (size_t)ring_rows * SC) + CS * sizeof(double);
     static_assert(W >= 32, "strip too narrow");
-    static_assert(2 * (NS - 1) + 1 + D + 2 <= CS, "c_n ring too short");
+    static_assert(2 * (NS - 1) + 1 + D + 1 <= 16, "c_n ring too short");
 };
 
 // active for an S-step launch: no budget, or at least S steps left (the host never issues an S-step launch
@@ -179,7 +179,7 @@ __device__ __forceinline__ void sweep_segment(const Layout& L, const int sys, co
     const int ipitch = L.pitch;
     const int adjH = col_valid ? col : 0;
     const int adjF = (szF ? cf : 0) + Y, adjF2 = ((i < 2 && szF2) ? cf2 : 0) + Y;
-    const int two = (i < 2) ? 1 : 0, first = (i == 0) ? 1 : 0;
+    const int two = (i < 2) ? 1 : 0;
 
     __syncthreads();   // the previous segment (or the scan) is done with the rings / sh
     if (i < NS + 2) sh.Es[i] = field_E(c, ((double)k + 0.5 * (double)i) * L.dt);   // (C14)
@@ -204,7 +204,7 @@ __device__ __forceinline__ void sweep_segment(const Layout& L, const int sys, co
             cp_async16_sz(sF + slot * FROW + i * 16, Hold + (o + adjF), in ? szF : 0);
             cp_async16_sz_if(sF + slot * FROW + (T + i) * 16, Hold + (o + adjF2), in ? szF2 : 0, two);
             if (v >= 1 && v <= Lr + 2 * NS - 2) cp_async16_sz(sH + slot * HROW + i * 16, Hold + (o + adjH), in ? szH : 0);
-            cp_async8_sz_if(sC + (unsigned)(v & (Cfg::CS - 1)) * 8, cn0 + (in ? row : 0), in ? 8 : 0, first);
+            cp_async8_sz_if(sC + (unsigned)((v & 15) + 16 * i) * 8, cn0 + (in ? row : 0), in ? 8 : 0, two);
         }
         cp_async_commit();
         off_in += ipitch;
@@ -232,9 +232,12 @@ __device__ __forceinline__ void sweep_segment(const Layout& L, const int sys, co
     const unsigned tF = sF + i * 16;
     constexpr unsigned tH_off = R * FROW, tQ_off = R * FROW + R * HROW;   // H ring, stage rings relative to tF
 
-    auto body = [&](auto edge_tag, const int u) {
+    // slot_tag: std::integral_constant<int, K>: K = u & 7 known at compile time (all ring offsets become
+    // immediates), or K = -1: taken from u at run time
+    auto body = [&](auto edge_tag, auto slot_tag, const int u) {
         constexpr bool EDGE = decltype(edge_tag)::value;
-        const unsigned su = (unsigned)(u & (R - 1));
+        constexpr int K = decltype(slot_tag)::value;
+        const unsigned su = K >= 0 ? (unsigned)K : (unsigned)(u & (R - 1));
         const unsigned o_u = su * FROW;                              // unit u  : arriving F^0 row
         const unsigned o_f = ((su + 5) & (R - 1)) * FROW;           // unit u-3: F^0 row of stage 1
         const unsigned o_h = ((su + 7) & (R - 1)) * HROW;           // unit u-1: H^0 row of stage 0
@@ -242,7 +245,10 @@ __device__ __forceinline__ void sweep_segment(const Layout& L, const int sys, co
         const unsigned q_w = su * SROW;                              // stage ring (depth 8): slot written now
         const unsigned q_p = ((su + 7) & (R - 1)) * SROW;           //   slot written one iteration ago
         const unsigned q_o = ((su + 4) & (R - 1)) * SROW;           //   slot written four iterations ago
-        const unsigned l_w = (unsigned)(u & 1) * SROW, l_p = SROW - l_w;   // last stage ring (depth 2)
+        const unsigned l_w = (su & 1u) * SROW, l_p = SROW - l_w;      // last stage ring (depth 2)
+        // c_n ring: unit v sits in slots v & 15 and (v & 15) + 16, so that unit u-1 and the NS-1 older ones
+        // (2 apart) are read at descending addresses from one base without wrap-around
+        const unsigned c_b = sC + (((su + 7) & (R - 1)) + ((unsigned)(u - 1) & 8u) + 16u) * 8;
         static_assert(QD == R, "stage ring slots share the input ring's slot arithmetic");
 
         cp_async_wait<D>();   // this thread's copies of unit u have landed
@@ -253,7 +259,8 @@ __device__ __forceinline__ void sweep_segment(const Layout& L, const int sys, co
             cp_async16_sz(tF + si * FROW, Hold + (off_in + adjF), szF);
             cp_async16_sz_if(tF + si * FROW + T * 16, Hold + (off_in + adjF2), szF2, two);
             cp_async16_sz(tF + tH_off + si * HROW, Hold + (off_in + adjH), szH);
-            cp_async8_sz_if(sC + (unsigned)((u + D + 1) & (Cfg::CS - 1)) * 8, cn0 + (row0 + D + 2), 8, first);
+            cp_async8_sz_if(sC + (((su + D + 1) & (R - 1)) + ((unsigned)(u + D + 1) & 8u) + 16u * i) * 8,
+                            cn0 + (row0 + D + 2), 8, two);
             cp_async_commit();
             off_in += ipitch;
         }
@@ -278,7 +285,7 @@ __device__ __forceinline__ void sweep_segment(const Layout& L, const int sys, co
             if (j == 0) ws[j] = lds_d2(tF + tH_off + o_h);
             else if (j == 1) ws[j] = lds_d2(tF + o_f + 16);
             else ws[j] = lds_d2(tF + tQ_off + (j - 2) * QD * SROW + q_o + 16);
-            cjs[j] = lds_d(sC + (unsigned)((u - 1 - 2 * j) & (Cfg::CS - 1)) * 8);   // unit u-1-2j = this row
+            cjs[j] = lds_d(c_b - 16 * j);                             // unit u-1-2j brought c of this row
         }
         // phase 2: the NS half-updates
 #pragma unroll
@@ -325,10 +332,25 @@ __device__ __forceinline__ void sweep_segment(const Layout& L, const int sys, co
     // (stage 0 within its rows, the prefetched unit u+D+1 a real row <= N of both input grids)
     const int u_steady_end = min(min(Lr + NS, Lr + 2 * NS - 3 - D), L.N - r0 + NS - D - 1);
     int u = u_start;
-    for (; u < min(3 * NS, n_iter); ++u) body(std::true_type{}, u);
-#pragma unroll 2
-    for (; u <= u_steady_end; ++u) body(std::false_type{}, u);
-    for (; u < n_iter; ++u) body(std::true_type{}, u);
+    using Dyn = std::integral_constant<int, -1>;
+    for (; u < min(3 * NS, n_iter); ++u) body(std::true_type{}, Dyn{}, u);
+    while (u <= u_steady_end) {
+        if ((u & 7) == 0 && u + 7 <= u_steady_end) {    // 8 iterations with compile-time ring slots
+            body(std::false_type{}, std::integral_constant<int, 0>{}, u);
+            body(std::false_type{}, std::integral_constant<int, 1>{}, u + 1);
+            body(std::false_type{}, std::integral_constant<int, 2>{}, u + 2);
+            body(std::false_type{}, std::integral_constant<int, 3>{}, u + 3);
+            body(std::false_type{}, std::integral_constant<int, 4>{}, u + 4);
+            body(std::false_type{}, std::integral_constant<int, 5>{}, u + 5);
+            body(std::false_type{}, std::integral_constant<int, 6>{}, u + 6);
+            body(std::false_type{}, std::integral_constant<int, 7>{}, u + 7);
+            u += 8;
+        } else {
+            body(std::false_type{}, Dyn{}, u);
+            ++u;
+        }
+    }
+    for (; u < n_iter; ++u) body(std::true_type{}, Dyn{}, u);
     cp_async_wait<0>();
 
     // per-strip partial sums of row 0 (a) and row 1 (b) of each of the S new whole grids -> eq. (12), (20)
