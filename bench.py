@@ -215,6 +215,8 @@ def run_ours(args):
         s.set_option("sweep_steps", args.sweep_steps)
     if args.ctas:
         s.set_option("sweep_ctas", args.ctas)
+    if args.res_ctas:
+        s.set_option("resident_ctas", args.res_ctas)
     s.init_equilibrium()
     s.step(max(3, args.warmup))
     barrier()
@@ -257,6 +259,8 @@ def run_ours(args):
         s2.set_option("sweep_steps", args.sweep_steps)
     if args.ctas:
         s2.set_option("sweep_ctas", args.ctas)
+    if args.res_ctas:
+        s2.set_option("resident_ctas", args.res_ctas)
     s2.init_equilibrium()
     s2.step(args.steps)
     obs2 = s2.observables()
@@ -326,10 +330,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--workload", type=int, default=4, help="BASELINE.json config index (default 4)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 split, 2 fused")
+    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 split, 2 fused tiles, 3 sweep, 4 resident")
     ap.add_argument("--tile-rows", type=int, default=0)
     ap.add_argument("--sweep-steps", type=int, default=0, help="steps fused per launch (0 auto)")
     ap.add_argument("--ctas", type=int, default=0, help="persistent CTAs of the sweep kernel (0 auto)")
+    ap.add_argument("--res-ctas", type=int, default=0, help="slabs of the resident kernel (0 auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

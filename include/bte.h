@@ -120,7 +120,13 @@ int bte_set_state(bte_ctx* ctx, int32_t system, int32_t grid_id, const double* a
 /* Tuning / variant selection, before or between bte_step calls.  Keys:
  *   "variant"      0 = automatic (default), 1 = two half-update kernels per step (96 B/point/step),
  *                  2 = fused whole+fractional kernel on a 2-D tile grid (64 B/point/step),
- *                  3 = persistent sweep kernel, S steps per launch (64/S B/point/step; the default path)
+ *                  3 = persistent sweep kernel, S steps per launch (64/S B/point/step; the default path
+ *                      for lattices larger than the GPU's shared memory),
+ *                  4 = resident kernel: the whole time loop of one bte_step call in ONE launch, state held
+ *                      in shared memory (n_batch = 1 and both grids must fit the shared memory of the GPU;
+ *                      otherwise variant 3 runs).  Automatic choice: 4 when usable and n_steps >= 4, else 3.
+ *   "resident_ctas" slabs (CTAs) of variant 4: 1 = one CTA, 2..16 = one thread-block cluster, more = cooperative
+ *                  grid; 0 = automatic
  *   "sweep_steps"  S of variant 3: 1..3, 0 = automatic
  *   "sweep_ctas"   CTAs of the persistent sweep kernel, 0 = SMs x resident CTAs
  *   "graph_steps"  launches captured per CUDA graph for launch-bound grids; 0 = plain launches, -1 = auto

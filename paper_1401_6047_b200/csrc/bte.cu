@@ -2,6 +2,7 @@
 // Product code: must not include, link or call anything under oracle/.
 #include "../../include/bte.h"
 #include "bte_sweep.cuh"
+#include "bte_resident.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -40,12 +41,23 @@ size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Offsets {
     int pitch;
-    size_t state, state_bytes, cn, gm, phi, sc, ss, partial, gctl, total;
+    size_t state, state_bytes, cn, gm, phi, sc, ss, partial, gctl, rhalo, rout, rflag, total;
 };
 
 bool grid_ok(const bte_grid* g) {
     return g && g->n_harm >= 1 && g->n_phiy >= 3 && g->n_batch >= 1 && g->n_batch <= 65535 &&
            g->n_harm < 65535 && g->dt > 0.0 && std::isfinite(g->dt);
+}
+
+// resident (on-chip) variant: at most RES_MAX_CTAS slabs; usable shared memory per CTA (227 KB minus the
+// kernel's static shared memory)
+constexpr int RES_MAX_CTAS = 148;
+constexpr size_t RES_SMEM_CAP = 227 * 1024 - 1024;
+
+bool resident_possible(const bte_grid* g) {
+    if (g->n_batch != 1) return false;
+    const int wc = (g->n_phiy + RES_MAX_CTAS - 1) / RES_MAX_CTAS;
+    return resident_smem_bytes(g->n_harm, wc) <= RES_SMEM_CAP;
 }
 
 Offsets offsets_for(const bte_grid* g) {
@@ -62,6 +74,11 @@ Offsets offsets_for(const bte_grid* g) {
     o.ss = off;      off = align_up(off + nb * sizeof(SysState));
     o.partial = off; off = align_up(off + (size_t)SWEEP_MAX_STEPS * nb * pitch * 2 * sizeof(double));
     o.gctl = off;    off = align_up(off + 64);
+    // resident variant: edge columns of both grids of every slab, per-slab sums
+    o.rhalo = off;
+    if (resident_possible(g)) off = align_up(off + (size_t)2 * RES_MAX_CTAS * 2 * (g->n_harm + 1) * sizeof(double2));
+    o.rout = off;    off = align_up(off + (size_t)RES_MAX_CTAS * 8 * sizeof(double));
+    o.rflag = off;   off = align_up(off + (size_t)RES_MAX_CTAS * sizeof(unsigned int));
     o.total = off;
     return o;
 }
@@ -83,7 +100,7 @@ void bessel_i_ratios(double x, int N, std::vector<double>& r) {
     for (int n = 0; n <= N; ++n) r[n] = t[n] / t[0];
 }
 
-enum Variant { VAR_AUTO = 0, VAR_SPLIT = 1, VAR_FUSED = 2, VAR_SWEEP = 3 };
+enum Variant { VAR_AUTO = 0, VAR_SPLIT = 1, VAR_FUSED = 2, VAR_SWEEP = 3, VAR_RESIDENT = 4 };
 
 }  // namespace
 
@@ -110,6 +127,11 @@ struct bte_ctx {
     int sw_grid[SWEEP_MAX_STEPS + 1];   // grid of the S-step kernel; 0 = not usable for this problem
     int sm_count;
     std::vector<int64_t> budgets;    // sorted distinct step budgets (n_steps_total > 0)
+    // resident (on-chip) kernel launch plan
+    int res_ctas_opt;                // option: slabs (0 = automatic)
+    int res_mode;                    // -1 = not usable; 0 one CTA, 1 one cluster, 2 cooperative grid
+    int res_G, res_Wc, res_T;
+    size_t res_smem;
     // CUDA graph cache
     cudaGraph_t graph;
     cudaGraphExec_t graph_exec;
@@ -205,9 +227,121 @@ int plan_sweep(bte_ctx* c) {
     return BTE_OK;
 }
 
+// ---- resident kernel: the whole time loop on chip (bte_resident.cuh) -------------------------------------
+void* resident_fn(int mode) {
+    return mode == 0 ? (void*)resident_kernel<0> : mode == 1 ? (void*)resident_kernel<1> : (void*)resident_kernel<2>;
+}
+
+// compute threads of a CTA (one more warp does the bookkeeping): one point per thread up to 31 warps
+int resident_threads(int rows, int wc) {
+    long long t = ((long long)rows * wc + 31) / 32 * 32;
+    if (t > 992) t = 992;
+    if (t < 64) t = 64;
+    return (int)t;
+}
+
+// Try one (mode, G) combination: shared memory fits and the launch shape is schedulable.
+bool resident_try(bte_ctx* c, int mode, int G) {
+    const int M1 = c->grid.n_phiy, N = c->grid.n_harm;
+    if (G < 1 || G > M1) return false;
+    const int wc = (M1 + G - 1) / G;
+    const int Ge = (M1 + wc - 1) / wc;          // slabs actually needed with this width
+    if ((mode == 0) != (Ge == 1)) return false;
+    if (mode == 1 && Ge != G) return false;    // cluster sizes are taken as given (2, 4, 8, 16)
+    const size_t smem = resident_smem_bytes(N, wc);
+    if (smem > RES_SMEM_CAP) return false;
+    void* fn = resident_fn(mode);
+    const int T = resident_threads(N + 1, wc);
+    if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    if (mode == 1) {
+        if (Ge > 8 && cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) {
+            cudaGetLastError();
+            return false;
+        }
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(Ge); cfg.blockDim = dim3(T + 32); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = Ge; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int nclusters = 0;
+        if (cudaOccupancyMaxActiveClusters(&nclusters, fn, &cfg) != cudaSuccess || nclusters < 1) {
+            cudaGetLastError();
+            return false;
+        }
+    } else if (mode == 2) {
+        int occ = 0, coop = 0, dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        if (!coop || cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, T + 32, smem) != cudaSuccess ||
+            (long long)occ * c->sm_count < Ge) {
+            cudaGetLastError();
+            return false;
+        }
+    }
+    c->res_mode = mode; c->res_G = Ge; c->res_Wc = wc; c->res_T = T; c->res_smem = smem;
+    return true;
+}
+
+int plan_resident(bte_ctx* c) {
+    c->res_mode = -1;
+    if (!resident_possible(&c->grid)) return BTE_OK;
+    const long long pts = (long long)(c->grid.n_harm + 1) * c->grid.n_phiy;
+    const int maxg = c->sm_count < RES_MAX_CTAS ? c->sm_count : RES_MAX_CTAS;
+    if (c->res_ctas_opt > 0) {                  // explicit slab count: 1 = one CTA, 2..16 = cluster, more = grid
+        const int G = c->res_ctas_opt;
+        if (G == 1) resident_try(c, 0, 1);
+        else if (G <= 16 && resident_try(c, 1, G)) {}
+        else if (G <= maxg) resident_try(c, 2, G);
+        return BTE_OK;
+    }
+    // automatic: the fewest slabs that leave about one point per thread (synchronisation cost grows with the
+    // number of CTAs: __syncthreads < cluster barrier < neighbour flags through L2)
+    if (pts <= 992 && resident_try(c, 0, 1)) return BTE_OK;
+    for (int G = 2; G <= 16; G *= 2)
+        if ((pts / G <= 992 || G == 16) && resident_try(c, 1, G)) return BTE_OK;
+    for (int G = 8; G >= 2; G /= 2)             // 16 not schedulable / does not fit: smaller clusters that fit
+        if (resident_try(c, 1, G)) return BTE_OK;
+    if (resident_try(c, 0, 1)) return BTE_OK;
+    resident_try(c, 2, maxg);
+    return BTE_OK;
+}
+
+int launch_resident(bte_ctx* c, int64_t n_steps) {
+    ResidentArgs A{};
+    A.G = c->res_G; A.Wc = c->res_Wc; A.T = c->res_T; A.n_steps = n_steps;
+    A.halo = (double2*)(c->ws + c->off.rhalo);
+    A.cta_out = (double*)(c->ws + c->off.rout);
+    A.flag = (unsigned int*)(c->ws + c->off.rflag);
+    void* fn = resident_fn(c->res_mode);
+    void* args[] = {&c->L, &A};
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(c->res_G); cfg.blockDim = dim3(c->res_T + 32); cfg.dynamicSmemBytes = c->res_smem;
+    cfg.stream = c->stream;
+    cudaLaunchAttribute at[1];
+    cfg.attrs = at; cfg.numAttrs = 0;
+    if (c->res_mode == 1) {
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = c->res_G; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.numAttrs = 1;
+    } else if (c->res_mode == 2) {
+        CUDA_TRY(cudaMemsetAsync(A.flag, 0, (size_t)c->res_G * sizeof(unsigned int), c->stream));
+        at[0].id = cudaLaunchAttributeCooperative;
+        at[0].val.cooperative = 1;
+        cfg.numAttrs = 1;
+    }
+    CUDA_TRY(cudaLaunchKernelExC(&cfg, fn, args));
+    c->launches += 1;
+    return BTE_OK;
+}
+
 int effective_variant(const bte_ctx* c) {
     if (c->variant == VAR_AUTO) return c->sw_grid[1] > 0 ? VAR_SWEEP : VAR_FUSED;
-    if (c->variant == VAR_SWEEP && c->sw_grid[1] == 0) return VAR_FUSED;
+    if ((c->variant == VAR_SWEEP || c->variant == VAR_RESIDENT) && c->sw_grid[1] == 0) return VAR_FUSED;
+    if (c->variant == VAR_RESIDENT) return VAR_SWEEP;   // what runs when the resident kernel is not used
     return c->variant;
 }
 
@@ -421,6 +555,7 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
     std::sort(c->budgets.begin(), c->budgets.end());
     c->budgets.erase(std::unique(c->budgets.begin(), c->budgets.end()), c->budgets.end());
     c->sweep_steps = 0; c->sweep_ctas = 0; c->sm_count = 0; c->graph_S = 0;
+    c->res_ctas_opt = 0; c->res_mode = -1; c->res_G = 0; c->res_Wc = 0; c->res_T = 0; c->res_smem = 0;
     for (int S = 0; S <= SWEEP_MAX_STEPS; ++S) c->sw_grid[S] = 0;
     c->steps_issued = 0; c->launches = 0;
     c->variant = VAR_AUTO; c->graph_steps = -1;
@@ -435,6 +570,8 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
         return fail(BTE_ECUDA, "cudaFuncSetAttribute failed: %s (is this an sm_100a device?)", cudaGetErrorString(e));
     }
     rc = plan_sweep(c);
+    if (rc != BTE_OK) { delete c; return rc; }
+    rc = plan_resident(c);
     if (rc != BTE_OK) { delete c; return rc; }
     *out = c;
     return BTE_OK;
@@ -456,6 +593,19 @@ int bte_step(bte_ctx* c, int64_t n_steps) {
     if (!c) return fail(BTE_EINVAL, "bte_step: NULL ctx");
     if (n_steps < 0) return fail(BTE_EINVAL, "bte_step: n_steps < 0");
     int64_t left = n_steps;
+    // lattices that fit on chip: ONE launch runs the whole time loop out of shared memory (automatic choice
+    // from 4 steps on -- below that the load/store of the state is not amortised)
+    if (c->res_mode >= 0 && (c->variant == VAR_RESIDENT || (c->variant == VAR_AUTO && n_steps >= 4))) {
+        const int64_t tot = c->params[0].n_steps_total;
+        int64_t n = n_steps;
+        if (tot > 0) n = std::min<int64_t>(n, std::max<int64_t>(0, tot - c->steps_issued));
+        if (n > 0) {
+            const int rc = launch_resident(c, n);
+            if (rc != BTE_OK) return rc;
+        }
+        c->steps_issued += n_steps;
+        return BTE_OK;
+    }
     const int S = sweep_steps(c);
     const int var = effective_variant(c);
     // launch-bound grids: replay a graph of glen launch groups of S steps each (not with step budgets:
@@ -558,7 +708,7 @@ int bte_set_state(bte_ctx* c, int32_t system, int32_t grid_id, const double* a, 
 int bte_set_option(bte_ctx* c, const char* key, int64_t value) {
     if (!c || !key) return fail(BTE_EINVAL, "bte_set_option: NULL argument");
     if (!strcmp(key, "variant")) {
-        if (value < 0 || value > 3) return fail(BTE_EINVAL, "variant must be 0, 1, 2 or 3");
+        if (value < 0 || value > 4) return fail(BTE_EINVAL, "variant must be 0, 1, 2, 3 or 4");
         c->variant = (int)value;
         drop_graph(c);
         return BTE_OK;
@@ -579,6 +729,11 @@ int bte_set_option(bte_ctx* c, const char* key, int64_t value) {
         c->sweep_ctas = (int)value;
         drop_graph(c);
         return plan_sweep(c);
+    }
+    if (!strcmp(key, "resident_ctas")) {   // slabs of the resident kernel: 1 = one CTA, 2..16 = cluster, more = grid
+        if (value < 0 || value > RES_MAX_CTAS) return fail(BTE_EINVAL, "resident_ctas must be in [0, %d]", RES_MAX_CTAS);
+        c->res_ctas_opt = (int)value;
+        return plan_resident(c);
     }
     if (!strcmp(key, "sweep_steps")) {   // leap-frog steps fused per launch of the sweep kernel (0 = automatic)
         if (value < 0 || value > SWEEP_MAX_STEPS) return fail(BTE_EINVAL, "sweep_steps must be in [0, %d]", SWEEP_MAX_STEPS);

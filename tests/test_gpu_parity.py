@@ -16,12 +16,12 @@ pytestmark = pytest.mark.gpu
 
 # name -> (variant, leap-frog steps fused per launch of the sweep kernel)
 VARIANTS = {"split": (1, 0), "fused": (2, 0), "sweep1": (3, 1), "sweep2": (3, 2), "sweep3": (3, 3),
-            "auto": (0, 0)}
+            "resident": (4, 0), "auto": (0, 0)}
 SWEEPS = ["sweep1", "sweep2", "sweep3"]
-ALL = ["split", "fused"] + SWEEPS
+ALL = ["split", "fused"] + SWEEPS + ["resident"]
 
 
-def gpu_solver(w, variant="auto", graph_steps=None, tile_rows=None, ctas=None):
+def gpu_solver(w, variant="auto", graph_steps=None, tile_rows=None, ctas=None, res_ctas=None):
     from paper_1401_6047_b200 import Solver
     s = Solver(w.grid, w.params)
     s.set_option("variant", VARIANTS[variant][0])
@@ -32,12 +32,15 @@ def gpu_solver(w, variant="auto", graph_steps=None, tile_rows=None, ctas=None):
         s.set_option("tile_rows", tile_rows)
     if ctas is not None:
         s.set_option("sweep_ctas", ctas)     # number of persistent CTAs of the sweep kernel
+    if res_ctas is not None:
+        s.set_option("resident_ctas", res_ctas)   # slabs of the resident kernel
     s.init_equilibrium()
     return s
 
 
-def check(w, n_steps, variant, systems=None, graph_steps=None, tile_rows=None, chunks=None, ctas=None):
-    s = gpu_solver(w, variant, graph_steps, tile_rows, ctas)
+def check(w, n_steps, variant, systems=None, graph_steps=None, tile_rows=None, chunks=None, ctas=None,
+          res_ctas=None):
+    s = gpu_solver(w, variant, graph_steps, tile_rows, ctas, res_ctas)
     if chunks:                      # several bte_step calls must equal one
         for c in chunks:
             s.step(c)
@@ -105,6 +108,41 @@ def test_sweep_partition_batched(ctas, variant):
         assert_obs_close(obs[i], sim.observables(), w.params[i], w.grid.dt, what=f"linbatch[{i}] ctas={ctas}")
 
 
+@pytest.mark.parametrize("res_ctas", [1, 2, 3, 4, 5, 8, 16, 17, 40, 148, 0])
+def test_resident_slabs(res_ctas):
+    """Resident kernel: one CTA, clusters of 2..16 CTAs (edge columns through distributed shared memory),
+    cooperative grids (edge columns through L2), ragged last slab; one launch per bte_step call."""
+    w = W.small_case(N=21, M1=300 if res_ctas != 1 else 150, dt=0.004, n_steps=17, avg_start=3)
+    s = gpu_solver(w, "resident", res_ctas=res_ctas)
+    n0 = s.launch_count()
+    s.step(9); s.step(1); s.step(7)
+    assert s.launch_count() - n0 == 3
+    obs = s.observables()
+    sim = oracle_run(w, 17)[0]
+    assert_state_close(s, sim, 0, what=f"resident ctas={res_ctas}")
+    assert_obs_close(obs[0], sim.observables(), w.params[0], w.grid.dt, what=f"resident ctas={res_ctas}")
+    s.destroy()
+
+
+def test_resident_interleaves_with_sweep_and_budget():
+    """The resident kernel and the streaming kernels share the state: alternate them; a step budget freezes
+    the system exactly at n_steps_total."""
+    w = W.small_case(N=12, M1=190, dt=0.004, n_steps=40, avg_start=5)
+    w.params[0].n_steps_total = 33
+    s = gpu_solver(w, "auto")
+    s.step(10)                          # resident (>= 4 steps)
+    s.set_option("variant", 3); s.step(3)
+    s.set_option("variant", 4); s.step(2)
+    s.set_option("variant", 1); s.step(5)
+    s.set_option("variant", 0); s.step(50)      # runs into the budget
+    obs = s.observables()
+    assert obs[0].step == 33
+    sim = oracle_run(w, 70)[0]
+    assert_state_close(s, sim, 0, what="resident/sweep interleaved")
+    assert_obs_close(obs[0], sim.observables(), w.params[0], w.grid.dt, what="resident/sweep interleaved")
+    s.destroy()
+
+
 @pytest.mark.parametrize("variant", ALL)
 def test_graph_replay_equals_plain_launches(variant):
     w = W.small_case(N=10, M1=140, n_steps=50, avg_start=7)
@@ -118,7 +156,7 @@ def test_fused_equals_split_bitwise_state():
     differ only in nothing -- same operation order -- so we ask for exact equality)."""
     w = W.small_case(N=14, M1=260, n_steps=31)
     a = gpu_solver(w, "split"); a.step(31)
-    for other in ["fused"] + SWEEPS:
+    for other in ["fused", "resident"] + SWEEPS:
         b = gpu_solver(w, other); b.step(31)
         for g in (0, 1):
             xa, xb = a.get_state(0, g)
