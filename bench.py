@@ -95,22 +95,7 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def dist_env():
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    return rank, world, local
-
-
-def replica_workload(index, rank):
-    """Rank r advances its own independent system: the batch of a parameter sweep sharded over ranks
-    (no data-path collective).  Rank r shifts E_dc slightly so the replicas are
-    distinct parameter points."""
-    w = W.get(index)
-    if rank > 0:
-        for p in w.params:
-            p.E_dc = p.E_dc + 0.01 * rank
-    return w
+from paper_1401_6047_b200.multi import dist_env, replica_workload, max_over_ranks as _max_over_ranks  # noqa: E402
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -199,11 +184,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return _max_over_ranks(x, dev)
 
     # ---- device-resident measurement: inputs (state) already in HBM ---------------------------------
     s = Solver(w.grid, w.params, device=dev)

@@ -1,0 +1,108 @@
+"""The C-ABI boundary without a GPU: libbte_b200.so loads, exports every symbol include/bte.h declares, and
+its argument validation (which runs before any CUDA call) behaves as the header says.  No compute calls."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "bte.h")
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_1401_6047_b200 import binding, build
+    return binding.load_library(build.build())
+
+
+def declared_functions():
+    text = open(HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)                 # drop comments
+    return sorted(set(re.findall(r"\b(bte_[a-z_]+)\s*\(", text)))
+
+
+def test_header_declares_the_five_north_star_calls():
+    names = declared_functions()
+    for n in ("bte_create", "bte_init_equilibrium", "bte_step", "bte_observables", "bte_destroy"):
+        assert n in names
+
+
+def test_every_declared_symbol_is_exported(lib):
+    from paper_1401_6047_b200 import binding
+    names = declared_functions()
+    assert len(names) >= 11
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in include/bte.h but not exported by libbte_b200.so"
+    assert sorted(binding.EXPORTS) == names, "binding.EXPORTS must list exactly the header's functions"
+
+
+def test_struct_layouts_match_header():
+    from paper_1401_6047_b200 import binding
+    assert C.sizeof(binding.bte_grid) == 24            # 4 x int32 + double
+    assert C.sizeof(binding.bte_params) == 9 * 8 + 2 * 8
+    assert C.sizeof(binding.bte_obs) == 8 + 8 * 8
+
+
+def test_workspace_bytes_is_a_pure_function(lib):
+    from paper_1401_6047_b200 import binding
+    lib.bte_workspace_bytes.restype = C.c_size_t
+    small = lib.bte_workspace_bytes(C.byref(binding.make_grid(20, 201, 1, 0.005)))
+    big = lib.bte_workspace_bytes(C.byref(binding.make_grid(512, 32001, 1, 0.001)))
+    assert 0 < small < big
+    # state: 2 buffers x 2 grids x (N + 1 + ghost rows) x pitch x 16 B dominates
+    assert big >= 2 * 2 * 513 * 32001 * 16 and big < 1.1 * 2 * 2 * 517 * 32008 * 16
+    assert lib.bte_workspace_bytes(C.byref(binding.make_grid(0, 201, 1, 0.005))) == 0      # N < 1
+    assert lib.bte_workspace_bytes(C.byref(binding.make_grid(20, 2, 1, 0.005))) == 0       # M+1 < 3
+    assert lib.bte_workspace_bytes(C.byref(binding.make_grid(20, 201, 0, 0.005))) == 0     # n_batch < 1
+    assert lib.bte_workspace_bytes(C.byref(binding.make_grid(20, 201, 1, 0.0))) == 0       # dt <= 0
+    assert lib.bte_workspace_bytes(None) == 0
+
+
+def _create(lib, grid, params, ws=0x10000, nbytes=1 << 40):
+    out = C.c_void_p()
+    rc = lib.bte_create(C.byref(grid), params, C.c_void_p(ws), C.c_size_t(nbytes), None, C.byref(out))
+    return rc, out
+
+
+def test_create_validates_before_touching_cuda(lib):
+    """Every rejection below happens in the argument checks of bte_create, i.e. before the first CUDA call,
+    so it can be exercised on a box without a GPU (the fake workspace pointer is never dereferenced)."""
+    from paper_1401_6047_b200 import binding, workloads as W
+    lib.bte_last_error.restype = C.c_char_p
+    w = W.small_case(N=4, M1=41, phiy_max=4.0)
+    g, ps = binding.make_grid(4, 41, 1, w.grid.dt), binding.make_params(w.params)
+    rc, out = _create(lib, g, ps, nbytes=16)
+    assert rc == -3 and not out.value and b"workspace" in lib.bte_last_error()             # BTE_ENOMEM
+    rc, out = _create(lib, g, ps, ws=0x10008)
+    assert rc == -3 and not out.value                                                       # misaligned
+    rc, out = _create(lib, g, None)
+    assert rc == -1 and not out.value                                                       # NULL params
+    bad = W.small_case(N=4, M1=41, mu=-1.0, phiy_max=4.0)
+    rc, out = _create(lib, g, binding.make_params(bad.params))
+    assert rc == -1 and not out.value                                                       # mu <= 0
+    bad = W.small_case(N=4, M1=41, dt=0.5, B=4.0, phiy_max=4.0)                             # |B| dt/dphi = 10
+    rc, out = _create(lib, binding.make_grid(4, 41, 1, 0.5), binding.make_params(bad.params))
+    assert rc == -2 and not out.value and b"unstable" in lib.bte_last_error()               # BTE_EUNSTABLE
+    assert lib.bte_step(None, 1) == -1 and lib.bte_destroy(None) == 0
+
+
+def test_product_path_fails_loudly_without_a_gpu():
+    """No CPU fallback: on a box without CUDA the public API raises instead of computing."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("CUDA present")
+    from paper_1401_6047_b200 import Solver, workloads as W
+    w = W.small_case()
+    with pytest.raises(Exception):
+        Solver(w.grid, w.params)
+
+
+def test_product_does_not_import_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1401_6047_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", text, flags=re.M), f
+                assert "bte_oracle" not in text, f
