@@ -234,9 +234,8 @@ def test_config0_full(variant):
     assert_obs_close(o, sim.observables(), w.params[0], w.grid.dt, what="config0")
 
 
-def test_config1_prefix_and_full_observables():
-    """Prefix of 3000 steps: full state parity.  Full length (62 832 steps): observables against the
-    oracle values stored in tests/golden/config1_full.json (written by tests/golden/make_golden.py)."""
+def test_config1_prefix():
+    """Prefix of 3000 steps: full state parity (full length: tests/test_gpu_full_size.py)."""
     w = W.config1()
     check(w, 3000, "auto")
 
