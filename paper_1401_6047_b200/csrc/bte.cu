@@ -599,9 +599,11 @@ int bte_step(bte_ctx* c, int64_t n_steps) {
         const int64_t tot = c->params[0].n_steps_total;
         int64_t n = n_steps;
         if (tot > 0) n = std::min<int64_t>(n, std::max<int64_t>(0, tot - c->steps_issued));
-        if (n > 0) {
-            const int rc = launch_resident(c, n);
+        while (n > 0) {                      // 32-bit half-update counters inside the kernel: <= 2^30 steps a launch
+            const int64_t m = std::min<int64_t>(n, (int64_t)1 << 30);
+            const int rc = launch_resident(c, m);
             if (rc != BTE_OK) return rc;
+            n -= m;
         }
         c->steps_issued += n_steps;
         return BTE_OK;

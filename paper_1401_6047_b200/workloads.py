@@ -185,6 +185,24 @@ def config4() -> Workload:
 CONFIGS = {0: config0, 1: config1, 2: config2, 3: config3, 4: config4}
 
 
+def absorption_sweep(omegas, E_dc: float, E_omega: float, B: float, mu: float, N: int, M1: int, dt: float,
+                     t_relax: float = 10.0, periods: int = 8, alpha: float = 1.0) -> Workload:
+    """The paper's use of the solver (Fig. 3, Fig. 4): one system per frequency omega_i, all
+    other parameters shared.  Each system relaxes until t_relax (the paper: t = 10), then the
+    running sums of eq. (17) cover an integer number of ac periods; the step budget ends the system there."""
+    ps = []
+    k_relax = int(round(t_relax / dt))
+    longest = 0
+    for w in omegas:
+        ext = phiy_extent(mu, E_dc, E_omega, B, dt, M1)
+        total = k_relax + steps_for_periods(periods, w, dt)
+        longest = max(longest, total)
+        ps.append(Params(E_dc=E_dc, E_omega=E_omega, omega=float(w), B=B, mu=mu, alpha=alpha, phiy_min=-ext,
+                         phiy_max=ext, kappa_scale=1.0, n_steps_total=total, avg_start_step=k_relax))
+    return Workload(name="absorption_sweep", grid=Grid(N, M1, len(ps), dt), params=ps, n_steps=longest,
+                    note=f"A(omega): relax to t = {t_relax}, then {periods} ac periods per system")
+
+
 def get(index: int) -> Workload:
     return CONFIGS[index]()
 

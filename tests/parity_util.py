@@ -53,3 +53,22 @@ def assert_obs_close(got, ref, p, dt, tol=TOL_OBS, what=""):
         assert abs(g - r) <= tol * max(abs(r), vf * win), f"{what}: {k} {g} vs {r}"
     assert abs(got.window - ref.window) <= 1e-12 * max(ref.window, dt), f"{what}: window"
     assert abs(got.edge_leak - ref.edge_leak) <= tol * max(abs(ref.edge_leak), vf), f"{what}: edge_leak"
+
+
+def tucker_averages(mu, E_dc, E_w, w, nmax=60):
+    """B = 0 closed forms, eq. (42)-(43) of the paper (L208-213) in eq. (17)'s normalisation (C9):
+    <v> = (I1/I0) sum_n J_n(b)^2 xi(E_dc + n w),  <v cos wt> = (I1/2I0) sum_n J_n(b)[J_{n+1}(b) + J_{n-1}(b)]
+    xi(E_dc + n w), b = E_w / w, xi(E) = E / (1 + E^2).  Returns (<v>, <v cos wt>, A = (2 I0/I1) <v cos wt>)."""
+    nn = np.arange(-nmax, nmax + 1)
+    beta = E_w / w
+    J, Jp, Jm = special.jv(nn, beta), special.jv(nn + 1, beta), special.jv(nn - 1, beta)
+    xi = (E_dc + nn * w) / (1 + (E_dc + nn * w) ** 2)
+    r = float(special.ive(1, mu) / special.ive(0, mu))
+    v_mean = r * float(np.sum(J * J * xi))
+    v_cos = 0.5 * r * float(np.sum(J * (Jp + Jm) * xi))
+    return v_mean, v_cos, 2.0 / r * v_cos
+
+
+def absorption(obs, mu):
+    """Eq. (17): A = (2 I0(mu)/I1(mu)) <v_dr cos wt>, from the raw sums the library returns (C9)."""
+    return 2.0 * float(special.ive(0, mu) / special.ive(1, mu)) * obs.sum_vcos_dt / obs.window

@@ -54,3 +54,26 @@ def test_updates_between_counts_frozen_systems_out():
     total = sum(p.n_steps_total for p in w.params) * pts
     assert w.updates_between(0, w.n_steps + 10) == total
     assert w.updates_between(0, 1) == 3 * pts
+
+
+def test_absorption_sweep_windows_are_whole_periods():
+    w = W.absorption_sweep([1.0, 2.5, 7.0], E_dc=5.0, E_omega=1.0, B=0.0, mu=50.0, N=6, M1=41, dt=0.002,
+                           periods=6)
+    assert w.grid.n_batch == 3 and w.n_steps == max(p.n_steps_total for p in w.params)
+    for p in w.params:
+        assert p.avg_start_step == 5000                                   # t = 10
+        n_avg = p.n_steps_total - p.avg_start_step
+        assert abs(n_avg * 0.002 - 6 * 2 * math.pi / p.omega) <= 0.002    # an integer number of periods
+
+
+def test_tucker_helper_against_the_oracle_on_cpu():
+    """The closed form used by the GPU spectrum test, checked here against the oracle at one frequency."""
+    from oracle import OracleSim
+    from parity_util import absorption, tucker_averages
+    w = W.absorption_sweep([3.0], E_dc=5.0, E_omega=1.0, B=0.0, mu=50.0, N=3, M1=21, dt=0.002, periods=6)
+    sim = OracleSim(3, 21, 0.002, w.params[0])
+    sim.init_equilibrium()
+    sim.step(w.n_steps)
+    A = absorption(sim.observables(), 50.0)
+    ref = tucker_averages(50.0, 5.0, 1.0, 3.0)[2]
+    assert abs(A - ref) < 2e-3 * max(abs(ref), 0.05)
