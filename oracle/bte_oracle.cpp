@@ -15,7 +15,7 @@
  * Esaki-Tsu-type steady drift velocity, norm conservation, relaxation to f0, the B=0 mirror symmetry,
  * the field-reversal mirror, E=0 stationarity of f0 with order-2 convergence, order-2 convergence in
  * dt, the Tucker ac averages, a dense brute-force restatement on tiny grids, checkerboard independence
- * and affinity.  Absolute values of configs 1-4 have no closed form and the paper prints none:
+ * and affinity; the reconstruction of f (eq. 8) against eq. (13) at t = 0 and against a numpy contraction.  Absolute values of configs 1-4 have no closed form and the paper prints none:
  * for those "parity unpinned" beyond the invariants listed above.
  *
  * Build: g++ -std=c++17 -O2 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).
@@ -272,6 +272,26 @@ void oracle_apply_T(void* h, int32_t target, double delta, double ta, double tb)
         apply_T(s, delta, s->ha.data(), s->hb.data(), s->fa.data(), s->fb.data(), ta, tb);
     else
         apply_T(s, delta, s->fa.data(), s->fb.data(), s->ha.data(), s->hb.data(), ta, tb);
+}
+
+/* The distribution function itself, eq. (8): f(phi_x, phi_y) = sum_n a_n cos(n phi_x) + b_n sin(n phi_x), written
+ * out as that sum (n ascending) on K equidistant phi_x = -pi + 2 pi i / K, i = 0..K-1, for every phi_y lattice
+ * point.  grid: 0 = whole, 1 = fractional.  f: K x (M+1) row-major, m fastest.  (pinned by
+ * eq. (13) at t = 0 in tests/test_oracle_pins.py.)                                                          */
+void oracle_reconstruct_pdf(void* h, int32_t grid, int32_t K, double* f) {
+    Sim* s = (Sim*)h;
+    const double PI = 3.14159265358979323846;
+    const double* a = grid == 0 ? s->ha.data() : s->fa.data();
+    const double* b = grid == 0 ? s->hb.data() : s->fb.data();
+    for (int i = 0; i < K; ++i) {
+        const double x = -PI + 2.0 * PI * i / K;
+        for (int m = 0; m < s->M1; ++m) {
+            double acc = 0.0;
+            for (int n = 0; n <= s->N; ++n)
+                acc += a[idx(s, n, m)] * std::cos(n * x) + b[idx(s, n, m)] * std::sin(n * x);
+            f[(size_t)i * s->M1 + m] = acc;
+        }
+    }
 }
 
 int32_t oracle_max_threads(void) {

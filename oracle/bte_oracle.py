@@ -54,6 +54,7 @@ def _load():
         lib.oracle_set_state.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
         lib.oracle_get_equilibrium.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         lib.oracle_apply_T.argtypes = [C.c_void_p, C.c_int32, C.c_double, C.c_double, C.c_double]
+        lib.oracle_reconstruct_pdf.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
         lib.oracle_max_threads.restype = C.c_int32
         _lib = lib
     return _lib
@@ -125,6 +126,12 @@ class OracleSim:
         a0 = np.empty(self.shape)
         _load().oracle_get_equilibrium(self._h, phi.ctypes.data, a0.ctypes.data)
         return phi, a0
+
+    def reconstruct_pdf(self, grid: int, n_phix: int):
+        """f(phi_x, phi_y) of eq. (8) on phi_x = -pi + 2 pi i / n_phix; returns (n_phix, n_phiy)."""
+        f = np.empty((n_phix, self.M1))
+        _load().oracle_reconstruct_pdf(self._h, grid, n_phix, f.ctypes.data)
+        return f
 
     def apply_T(self, target: int, delta: float, ta: float, tb: float):
         _load().oracle_apply_T(self._h, target, delta, ta, tb)

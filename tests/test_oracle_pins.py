@@ -448,3 +448,41 @@ def test_frozen_system_stops_at_budget():
     o2 = s.observables()
     assert o2.step == 25 and np.array_equal(a1, s.get_state(0)[0])
     assert o1.sum_v_dt == o2.sum_v_dt and abs(o2.window - 15 * 0.01) < 1e-12
+
+
+# ---------------------------------------------------------------------------------------------------
+# NEXT-3: reconstruction of f(phi_x, phi_y), eq. (8)
+# ---------------------------------------------------------------------------------------------------
+def test_pdf_reconstruction_at_t0_is_eq13():
+    """At t = 0 the state is the equilibrium, so the reconstructed f must be the Boltzmann distribution as
+    printed in eq. (13) (up to the truncation at N harmonics: I_N(mu)/I_0(mu) ~ 1e-17 for mu = 2, N = 24)."""
+    mu, alpha, N, M1, K = 2.0, 0.9496, 24, 65, 48
+    s, p = make(N, M1, 0.01, mu=mu, alpha=alpha, phiy_min=-4.0, phiy_max=4.0)
+    s.init_equilibrium()
+    f = s.reconstruct_pdf(0, K)
+    phi, _ = s.equilibrium()
+    x = -np.pi + 2 * np.pi * np.arange(K) / K
+    want = (1.0 / (2 * np.pi * special.ive(0, mu))) * math.sqrt(mu / (2 * np.pi * alpha)) * \
+        np.exp(mu * (np.cos(x)[:, None] - 1.0) - 0.5 * mu * phi[None, :] ** 2)
+    assert f.shape == (K, M1)
+    assert np.abs(f - want).max() <= 1e-14 * want.max()
+    # and it integrates to 1: sqrt(alpha) int int f dphi_x dphi_y = 1, eq. (6)
+    dphi = phi[1] - phi[0]
+    assert abs(math.sqrt(alpha) * f.sum() * (2 * np.pi / K) * dphi - 1.0) < 1e-6   # phi_y cut at +-4
+
+
+def test_pdf_reconstruction_is_the_fourier_sum_of_any_state():
+    """Random state with sine terms: compare with a numpy contraction over n (b_n sin(n phi_x) included, sign
+    and the phi_x origin at -pi)."""
+    rng = np.random.default_rng(11)
+    N, M1, K = 5, 7, 16
+    s, _ = make(N, M1, 0.01, phiy_min=-1.0, phiy_max=1.0)
+    a, b = rng.standard_normal((N + 1, M1)), rng.standard_normal((N + 1, M1))
+    b[0] = 0.0
+    s.set_state(1, a, b)
+    f = s.reconstruct_pdf(1, K)
+    x = -np.pi + 2 * np.pi * np.arange(K) / K
+    n = np.arange(N + 1)
+    want = np.einsum("in,nm->im", np.cos(np.outer(x, n)), a) + np.einsum("in,nm->im", np.sin(np.outer(x, n)), b)
+    assert np.abs(f - want).max() <= 1e-13
+    assert abs(f[K // 2, 3] - a[:, 3].sum()) <= 1e-13            # phi_x = 0: cos = 1, sin = 0
