@@ -117,6 +117,13 @@ int bte_destroy(bte_ctx* ctx);
 int bte_get_state(bte_ctx* ctx, int32_t system, int32_t grid_id, double* a, double* b);
 int bte_set_state(bte_ctx* ctx, int32_t system, int32_t grid_id, const double* a, const double* b);
 
+/* The distribution function itself, eq. (8) (L63-64): f(phi_x, phi_y_m) = sum_n a_{n,m} cos(n phi_x) + b_{n,m} sin(n phi_x)
+ * of one system and grid on n_phix equidistant points phi_x_i = -pi + 2 pi i / n_phix, i = 0 .. n_phix-1 (the content
+ * of the paper's Fig. 2 and Fig. 5, as a headless buffer).
+ *   f : DEVICE, caller-owned, n_phix * n_phiy doubles, row-major [i][m], m fastest.  1 <= n_phix <= 2048.
+ * Reads the step counter's buffer flag (synchronises the stream once), then runs asynchronously on the stream. */
+int bte_reconstruct_pdf(bte_ctx* ctx, int32_t system, int32_t grid_id, int32_t n_phix, double* f /* device */);
+
 /* Tuning / variant selection, before or between bte_step calls.  Keys:
  *   "variant"      0 = automatic (default), 1 = two half-update kernels per step (96 B/point/step),
  *                  2 = fused whole+fractional kernel on a 2-D tile grid (64 B/point/step),

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libbte_b200.so")
 BTE_OK, BTE_EINVAL, BTE_EUNSTABLE, BTE_ENOMEM, BTE_ECUDA = 0, -1, -2, -3, -4
 
 EXPORTS = ("bte_workspace_bytes", "bte_create", "bte_init_equilibrium", "bte_step", "bte_observables",
-           "bte_destroy", "bte_get_state", "bte_set_state", "bte_set_option", "bte_launch_count",
+           "bte_destroy", "bte_get_state", "bte_set_state", "bte_reconstruct_pdf", "bte_set_option", "bte_launch_count",
            "bte_last_error")
 
 
@@ -86,6 +86,8 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.bte_get_state.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
     lib.bte_set_state.restype = C.c_int
     lib.bte_set_state.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
+    lib.bte_reconstruct_pdf.restype = C.c_int
+    lib.bte_reconstruct_pdf.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p]
     lib.bte_set_option.restype = C.c_int
     lib.bte_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_int64]
     lib.bte_launch_count.restype = C.c_int
@@ -191,6 +193,14 @@ class Solver:
         assert a.shape == self.shape and b.shape == self.shape
         _check(self._lib.bte_set_state(self._h, system, grid_id, C.c_void_p(a.ctypes.data),
                                        C.c_void_p(b.ctypes.data)))
+
+    def reconstruct_pdf(self, system: int, grid_id: int, n_phix: int):
+        """f(phi_x, phi_y) of eq. (8) on phi_x = -pi + 2 pi i / n_phix: a (n_phix, n_phiy) float64 tensor on the
+        solver's device, written by the library's kernel on the solver's stream."""
+        import torch
+        f = torch.empty((n_phix, self.shape[1]), dtype=torch.float64, device=self.workspace.device)
+        _check(self._lib.bte_reconstruct_pdf(self._h, system, grid_id, n_phix, C.c_void_p(f.data_ptr())))
+        return f
 
     def set_option(self, key: str, value: int):
         _check(self._lib.bte_set_option(self._h, key.encode(), int(value)))

@@ -707,6 +707,24 @@ int bte_set_state(bte_ctx* c, int32_t system, int32_t grid_id, const double* a, 
     return BTE_OK;
 }
 
+int bte_reconstruct_pdf(bte_ctx* c, int32_t system, int32_t grid_id, int32_t n_phix, double* f) {
+    if (!c || !f) return fail(BTE_EINVAL, "bte_reconstruct_pdf: NULL argument");
+    if (system < 0 || system >= c->grid.n_batch || grid_id < 0 || grid_id > 1)
+        return fail(BTE_EINVAL, "bte_reconstruct_pdf: bad system or grid index");
+    if (n_phix < 1 || n_phix > 2048) return fail(BTE_EINVAL, "bte_reconstruct_pdf: n_phix must be in [1, 2048]");
+    const int rows = c->grid.n_harm + 1, M1 = c->grid.n_phiy, pitch = c->off.pitch;
+    int buf = 0;
+    { const int rc = live_buffer(c, system, &buf); if (rc != BTE_OK) return rc; }
+    const size_t gp = (size_t)(rows + 2 * GHOST) * pitch, row0 = (size_t)GHOST * pitch;
+    const double2* z = c->L.state + (((size_t)buf * 2 + grid_id) * c->grid.n_batch + system) * gp + row0;
+    constexpr int KT = 16;
+    const dim3 g((unsigned)((M1 + 127) / 128), (unsigned)((n_phix + KT - 1) / KT));
+    pdf_kernel<KT><<<g, 128, 2 * (size_t)n_phix * sizeof(double), c->stream>>>(z, f, rows, M1, pitch, n_phix);
+    CUDA_TRY(cudaGetLastError());
+    c->launches += 1;
+    return BTE_OK;
+}
+
 int bte_set_option(bte_ctx* c, const char* key, int64_t value) {
     if (!c || !key) return fail(BTE_EINVAL, "bte_set_option: NULL argument");
     if (!strcmp(key, "variant")) {

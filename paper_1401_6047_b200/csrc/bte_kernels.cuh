@@ -390,4 +390,41 @@ __global__ void interleave_kernel(double2* __restrict__ z, const double* __restr
     z[(size_t)n * pitch + m] = w;
 }
 
+// ------------------------------------------------------------------------------------------------
+// the distribution function itself: f(phi_x, phi_y) = sum_n a_n cos(n phi_x) + b_n sin(n phi_x)
+// (eq. 8) on K equidistant phi_x_i = -pi + 2 pi i / K, for every phi_y lattice point; f is [K][M1], m fastest.
+// n phi_x_i = -n pi + 2 pi (n i mod K) / K exactly, so cos(n phi_x_i) = (-1)^n cos(2 pi j / K) with j = n i mod K
+// kept in integers: one K-entry table per CTA, no argument reduction error however large n is.
+// Thread = one phi_y column x KT values of phi_x; rows are read coalesced, each (a, b) once per KT outputs.
+// ------------------------------------------------------------------------------------------------
+template <int KT>
+__global__ void __launch_bounds__(128) pdf_kernel(const double2* __restrict__ z, double* __restrict__ f, int rows,
+                                                  int M1, int pitch, int K) {
+    extern __shared__ double tab[];          // cos(2 pi j / K), sin(2 pi j / K), j = 0..K-1
+    double* cs = tab;
+    double* sn = tab + K;
+    for (int j = threadIdx.x; j < K; j += blockDim.x) sincospi(2.0 * (double)j / (double)K, sn + j, cs + j);
+    __syncthreads();
+    const int m = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i0 = blockIdx.y * KT;
+    if (m >= M1) return;
+    double acc[KT];
+    int jn[KT];                              // n * i mod K
+#pragma unroll
+    for (int t = 0; t < KT; ++t) { acc[t] = 0.0; jn[t] = 0; }
+    for (int n = 0; n < rows; ++n) {
+        double2 w = z[(size_t)n * pitch + m];
+        if (n & 1) { w.x = -w.x; w.y = -w.y; }            // (-1)^n
+#pragma unroll
+        for (int t = 0; t < KT; ++t) {
+            acc[t] = __fma_rn(w.x, cs[jn[t]], __fma_rn(w.y, sn[jn[t]], acc[t]));
+            jn[t] += (i0 + t < K) ? i0 + t : 0;             // chunk tail beyond K: index stays 0, value unused
+            if (jn[t] >= K) jn[t] -= K;
+        }
+    }
+#pragma unroll
+    for (int t = 0; t < KT; ++t)
+        if (i0 + t < K) f[(size_t)(i0 + t) * M1 + m] = acc[t];
+}
+
 }  // namespace bte

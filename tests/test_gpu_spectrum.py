@@ -49,3 +49,24 @@ def test_absorption_spectrum_crossed_fields_against_oracle():
         assert_state_close(s, sim, i, what=f"A(omega) crossed[{i}]")
         assert_obs_close(obs[i], sim.observables(), w.params[i], w.grid.dt, what=f"A(omega) crossed[{i}]")
     s.destroy()
+
+
+@pytest.mark.parametrize("N,M1,K", [(6, 41, 16), (20, 300, 64), (33, 129, 37), (150, 500, 128)])
+def test_pdf_reconstruction_matches_oracle(N, M1, K):
+    """f(phi_x, phi_y) of eq. (8) from the evolved state, both grids, against the oracle's
+    plain Fourier sum; odd K and K not a multiple of the per-thread chunk included."""
+    from paper_1401_6047_b200 import Solver
+    from oracle import OracleSim
+    w = W.small_case(N=N, M1=M1, dt=0.004, n_steps=9, avg_start=2)
+    s = Solver(w.grid, w.params)
+    s.init_equilibrium()
+    s.step(9)
+    sim = OracleSim(N, M1, w.grid.dt, w.params[0])
+    sim.init_equilibrium()
+    sim.step(9)
+    for g in (0, 1):
+        f = s.reconstruct_pdf(0, g, K).cpu().numpy()
+        ref = sim.reconstruct_pdf(g, K)
+        assert f.shape == ref.shape == (K, M1)
+        assert np.abs(f - ref).max() <= 1e-12 * np.abs(ref).max()
+    s.destroy()
