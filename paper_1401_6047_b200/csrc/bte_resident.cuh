@@ -63,29 +63,45 @@ __host__ __device__ inline size_t resident_smem_bytes(int N, int Wc) {
     return 2 * rows * P * sizeof(double2) + (2 * (size_t)Wc + (size_t)N + 1) * sizeof(double);
 }
 
-// One application of T (eq. 38) at point (n, j) of the slab: X updated in place with the stencil of Sg.
-// Returns the new pair.  Both arrays are [(N+3)][P] with ghost rows and halo columns, so no predicates.
-__device__ __forceinline__ double2 resident_point(double2* X, const double2* Sg, int n, int j, int P,
-                                                  const double* phs, const double* gdts, const double* cns,
-                                                  const SysConst& c, const Layout& L, double Ea, double Eb) {
-    const int idx = (n + 1) * P + (j + 1);
+__device__ __forceinline__ double2 rlds_d2(unsigned addr) {
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];\n" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void rsts_d2(unsigned addr, double2 v) {
+    asm volatile("st.shared.v2.f64 [%0], {%1, %2};\n" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory");
+}
+__device__ __forceinline__ double rlds_d(unsigned addr) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];\n" : "=d"(v) : "r"(addr));
+    return v;
+}
+
+// One application of T (eq. 38) at point (n, j) of the slab: X updated in place with the stencil of S.
+// Returns the new pair.  sX, sS: shared-memory addresses of the two arrays, both [(N+3)][P] with ghost rows and
+// halo columns (no predicates); PB = P * 16 bytes; sph, sgdt, scn: addresses of the ph, gdt, c_n tables.
+__device__ __forceinline__ double2 resident_point(unsigned sX, unsigned sS, int n, int j, unsigned PB, unsigned sph,
+                                                  unsigned sgdt, unsigned scn, const SysConst& c, const Layout& L,
+                                                  double Ea, double Eb) {
+    const unsigned off = (unsigned)(n + 1) * PB + (unsigned)(j + 1) * 16;
+    const unsigned up = sS + off - PB, dn = sS + off + PB;
     double2 lo, hi;
     {
-        const double2 l = Sg[idx - P - 1], r = Sg[idx - P + 1];
+        const double2 l = rlds_d2(up - 16), r = rlds_d2(up + 16);
         lo.x = __dsub_rn(r.x, l.x); lo.y = __dsub_rn(r.y, l.y);
         if (n == 1) lo.x *= 2.0;                   // chi(1) = 2, eq. (11)
     }
     {
-        const double2 l = Sg[idx + P - 1], r = Sg[idx + P + 1];
+        const double2 l = rlds_d2(dn - 16), r = rlds_d2(dn + 16);
         hi.x = __dsub_rn(r.x, l.x); hi.y = __dsub_rn(r.y, l.y);
     }
-    const double ph = phs[j];
+    const double ph = rlds_d(sph + (unsigned)j * 8);
     const double hba = __dmul_rn(__fma_rn(c.B, ph, Ea), L.hd);
     const double hbb = __dmul_rn(__fma_rn(c.B, ph, Eb), L.hd);
-    double2 out = cn_point(X[idx], lo, hi, (double)n, hba, hbb, __dmul_rn(cns[n], gdts[j]), c.kappa_dt, L.xi, L.nu,
-                           L.nu2);
+    const double src = __dmul_rn(rlds_d(scn + (unsigned)n * 8), rlds_d(sgdt + (unsigned)j * 8));
+    double2 out = cn_point(rlds_d2(sX + off), lo, hi, (double)n, hba, hbb, src, c.kappa_dt, L.xi, L.nu, L.nu2);
     if (n == 0) out.y = 0.0;                       // b_0 == 0 (eq. 23, C3)
-    X[idx] = out;
+    rsts_d2(sX + off, out);
     return out;
 }
 
@@ -96,7 +112,6 @@ __global__ void __launch_bounds__(1024, 1) resident_kernel(const __grid_constant
     // tables filled 32 entries at a time by the service warp, far ahead of their use (rings of 64):
     __shared__ double Es[64];             // E at half-step q of this launch (time (2 k0 + q) dt/2)       (C14)
     __shared__ double Cs[64], Sn[64];     // cos, sin of omega t at step s of this launch (t = (k0+s+1) dt) (C9)
-    __shared__ double red[32][2];         // per-warp sums of a_{0,m}, b_{1,m} of the newest whole grid
     const int tid = threadIdx.x, T = A.T, NT = blockDim.x;
     const bool service = tid >= T;        // last warp: tables and the running sums, no lattice points
     const int lane = tid & 31, warp = tid >> 5;
@@ -146,7 +161,6 @@ __global__ void __launch_bounds__(1024, 1) resident_kernel(const __grid_constant
         if (e < 64) Es[e] = E_at(e);
         else csn_at(e - 64);
     }
-    if (tid < 32) { red[tid][0] = 0.0; red[tid][1] = 0.0; }
     __syncthreads();
 
     // this thread's points.  Edge columns (j = 0 and j = Wv-1) first: e = tid, tid + T, ... < nE;
@@ -160,13 +174,9 @@ __global__ void __launch_bounds__(1024, 1) resident_kernel(const __grid_constant
     // critical path of every half-update) to save four registers
     asm volatile("" : "+r"(n_first), "+r"(j_first), "+r"(dn), "+r"(dj));
     const unsigned sH = (unsigned)__cvta_generic_to_shared(Hs), sF = (unsigned)__cvta_generic_to_shared(Fs);
-    // does any lane of this warp own a point of row 0 or row 1 (the rows eq. 12 and eq. 20 sum over)?
-    bool mine = false;
-    if (!service) {
-        for (int e = tid; e < nE; e += T) mine = mine || (e - (e >= rows ? rows : 0)) <= 1;
-        mine = mine || (tid < 2 * Wi);            // interior points p = n * Wi + (j - 1) with n <= 1
-    }
-    const bool contributes = __any_sync(0xffffffffu, mine);
+    const unsigned PB = (unsigned)P * 16;
+    const unsigned sph = (unsigned)__cvta_generic_to_shared(phs), sgdt = (unsigned)__cvta_generic_to_shared(gdts),
+                   scn = (unsigned)__cvta_generic_to_shared(cns);
 
     // service lane 0: this slab's share of the observables (fixed order in k => deterministic)
     double A_last = 0.0, B_last = 0.0, SV = 0.0, SC = 0.0, SS = 0.0;
@@ -175,13 +185,17 @@ __global__ void __launch_bounds__(1024, 1) resident_kernel(const __grid_constant
     for (long long q = 0; q < 2 * A.n_steps; ++q) {
         const bool whole = (q & 1) == 0;
         double2* X = whole ? Hs : Fs;
-        const double2* Sg = whole ? Fs : Hs;
         const unsigned done = (unsigned)q + 1u;
         if (service) {
             if (q > 0 && (q & 31) == 0) Es[(q + 32 + lane) & 63] = E_at(q + 32 + lane);
             if (!whole) {                          // the whole grid of step s was finished one phase ago
                 const long long s = q >> 1;
-                double sa = red[lane][0], sb = red[lane][1];
+                // sums of eq. (12), (20) over this slab, read from the whole grid (not written in this phase)
+                double sa = 0.0, sb = 0.0;
+                for (int j = lane; j < Wv; j += 32) {
+                    sa += rlds_d2(sH + PB + (unsigned)(j + 1) * 16).x;          // a_{0,m}
+                    sb += rlds_d2(sH + 2 * PB + (unsigned)(j + 1) * 16).y;      // b_{1,m}
+                }
                 sa = warp_sum(sa); sb = warp_sum(sb);
                 if (lane == 0) {
                     A_last = sa; B_last = sb;
@@ -193,18 +207,13 @@ __global__ void __launch_bounds__(1024, 1) resident_kernel(const __grid_constant
                 if (s > 0 && (s & 31) == 0) csn_at(s + 32 + lane);
             }
         } else {
-            const unsigned sX = whole ? sH : sF;
+            const unsigned sX = whole ? sH : sF, sS = whole ? sF : sH;
             const double Ea = Es[q & 63], Eb = Es[(q + 2) & 63];
-            double acc_a = 0.0, acc_b = 0.0;
             // slab-edge columns first: their new values go to the neighbours' halo columns
             for (int e = tid; e < nE; e += T) {
                 const int side = e >= rows ? 1 : 0, n = e - side * rows;
                 const int j = side ? Wv - 1 : 0;
-                const double2 out = resident_point(X, Sg, n, j, P, phs, gdts, cns, c, L, Ea, Eb);
-                if (whole) {
-                    if (n == 0) acc_a += out.x;
-                    if (n == 1) acc_b += out.y;
-                }
+                const double2 out = resident_point(sX, sS, n, j, PB, sph, sgdt, scn, c, L, Ea, Eb);
                 if (MODE == 1) {
                     if (j == 0 && g > 0)
                         st_cluster_d2(cluster_map(sX + (unsigned)((n + 1) * P + Wc + 1) * 16, g - 1), out);
@@ -224,17 +233,9 @@ __global__ void __launch_bounds__(1024, 1) resident_kernel(const __grid_constant
             }
             int n = n_first, j = j_first;
             for (int p = tid; p < nI; p += T) {
-                const double2 out = resident_point(X, Sg, n, j + 1, P, phs, gdts, cns, c, L, Ea, Eb);
-                if (whole) {
-                    if (n == 0) acc_a += out.x;
-                    if (n == 1) acc_b += out.y;
-                }
+                resident_point(sX, sS, n, j + 1, PB, sph, sgdt, scn, c, L, Ea, Eb);
                 j += dj; n += dn;
                 if (j >= wi) { j -= wi; ++n; }
-            }
-            if (whole && contributes) {            // per-warp sums of row 0 (a) and row 1 (b)
-                acc_a = warp_sum(acc_a); acc_b = warp_sum(acc_b);
-                if (lane == 0) { red[warp][0] = acc_a; red[warp][1] = acc_b; }
             }
             if (MODE == 2) {
                 // halo columns of X for the next half-update, fetched in chunks of 32 rows: chunk ch < nch is rows
