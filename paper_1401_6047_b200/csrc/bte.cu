@@ -116,7 +116,7 @@ struct bte_ctx {
     // options
     int variant;
     int64_t graph_steps;    // -1 auto, 0 off
-    int tile_cols, tile_rows, prefetch_rows;
+    int tile_rows;
     // fused (tile grid) launch plan
     int rows_per_chunk;
     dim3 fgrid;
@@ -559,7 +559,7 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
     for (int S = 0; S <= SWEEP_MAX_STEPS; ++S) c->sw_grid[S] = 0;
     c->steps_issued = 0; c->launches = 0;
     c->variant = VAR_AUTO; c->graph_steps = -1;
-    c->tile_cols = 0; c->tile_rows = 0; c->prefetch_rows = 0;
+    c->tile_rows = 0;
     c->graph = nullptr; c->graph_exec = nullptr; c->graph_len = 0; c->graph_variant = 0;
     int rc = plan_fused(c);
     if (rc != BTE_OK) { delete c; return rc; }
@@ -744,7 +744,7 @@ int bte_set_option(bte_ctx* c, const char* key, int64_t value) {
         drop_graph(c);
         return plan_fused(c);
     }
-    if (!strcmp(key, "sweep_ctas") || !strcmp(key, "tile_cols")) {   // CTAs of the persistent sweep kernel (0 = SMs x occupancy)
+    if (!strcmp(key, "sweep_ctas")) {   // CTAs of the persistent sweep kernel (0 = SMs x occupancy)
         if (value < 0 || value > 65535) return fail(BTE_EINVAL, "%s must be in [0, 65535]", key);
         c->sweep_ctas = (int)value;
         drop_graph(c);
@@ -759,10 +759,6 @@ int bte_set_option(bte_ctx* c, const char* key, int64_t value) {
         if (value < 0 || value > SWEEP_MAX_STEPS) return fail(BTE_EINVAL, "sweep_steps must be in [0, %d]", SWEEP_MAX_STEPS);
         c->sweep_steps = (int)value;
         drop_graph(c);
-        return BTE_OK;
-    }
-    if (!strcmp(key, "prefetch_rows")) {
-        if (value != 0) return fail(BTE_EINVAL, "%s: only 0 (automatic) is supported in this build", key);
         return BTE_OK;
     }
     return fail(BTE_EINVAL, "bte_set_option: unknown key '%s'", key);
