@@ -198,6 +198,8 @@ def run_ours(args):
         s.set_option("sweep_ctas", args.ctas)
     if args.res_ctas:
         s.set_option("resident_ctas", args.res_ctas)
+    if args.sweep_threads:
+        s.set_option("sweep_threads", args.sweep_threads)
     s.init_equilibrium()
     s.step(max(3, args.warmup))
     barrier()
@@ -259,6 +261,8 @@ def run_ours(args):
             sol.set_option("sweep_ctas", args.ctas)
         if args.res_ctas:
             sol.set_option("resident_ctas", args.res_ctas)
+        if args.sweep_threads:
+            sol.set_option("sweep_threads", args.sweep_threads)
 
     nb, shape = w.grid.n_batch, (w.grid.n_harm + 1, w.grid.n_phiy)
     host_in = torch.empty((nb, 2, 2) + shape, dtype=torch.float64).pin_memory()
@@ -358,6 +362,7 @@ def main():
     ap.add_argument("--tile-rows", type=int, default=0)
     ap.add_argument("--sweep-steps", type=int, default=0, help="steps fused per launch (0 auto)")
     ap.add_argument("--ctas", type=int, default=0, help="persistent CTAs of the sweep kernel (0 auto)")
+    ap.add_argument("--sweep-threads", type=int, default=0, help="threads per CTA of the sweep kernel (0 auto)")
     ap.add_argument("--res-ctas", type=int, default=0, help="slabs of the resident kernel (0 auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -124,6 +124,7 @@ struct bte_ctx {
     bool has_budgets;
     int sweep_steps;                 // option: 0 = automatic, 1..SWEEP_MAX_STEPS
     int sweep_ctas;                  // option: grid-size override (0 = SMs x resident CTAs)
+    int sweep_threads;               // option: 0 = automatic, 128, 256
     int sw_grid[SWEEP_MAX_STEPS + 1];   // grid of the S-step kernel; 0 = not usable for this problem
     int sm_count;
     std::vector<int64_t> budgets;    // sorted distinct step budgets (n_steps_total > 0)
@@ -174,24 +175,40 @@ int plan_fused(bte_ctx* c) {
 // resident CTAs per SM the register budget of each instantiation is compiled for
 template <int S> struct SweepMinB { static constexpr int v = S == 1 ? 4 : S == 2 ? 3 : 2; };
 
-struct SweepFn { void* fn; size_t smem; int W; };
+struct SweepFn { void* fn; size_t smem; int W; int T; };
 
-template <int S>
-SweepFn sweep_fn_s(bool budgets) {
-    using Cfg = SweepCfg<FT, S>;
-    constexpr int MB = SweepMinB<S>::v;
-    return {budgets ? (void*)sweep_kernel<FT, S, true, MB> : (void*)sweep_kernel<FT, S, false, MB>,
-            Cfg::smem_bytes, Cfg::W};
+// T = 128 threads per CTA (several CTAs per SM) or T = 256 (half the strip-halo overhead, longer DRAM bursts
+// per row; S = 3 then runs one CTA per SM)
+template <int T, int S>
+SweepFn sweep_fn_ts(bool budgets) {
+    using Cfg = SweepCfg<T, S>;
+    constexpr int MB = T == 128 ? SweepMinB<S>::v : (S == 1 ? 2 : 1);
+    return {budgets ? (void*)sweep_kernel<T, S, true, MB> : (void*)sweep_kernel<T, S, false, MB>,
+            Cfg::smem_bytes, Cfg::W, T};
 }
 
-SweepFn sweep_fn(int S, bool budgets) {
+SweepFn sweep_fn(int S, bool budgets, bool wide) {
+    if (wide) {
+        switch (S) {
+            case 1: return sweep_fn_ts<256, 1>(budgets);
+            case 2: return sweep_fn_ts<256, 2>(budgets);
+            default: return sweep_fn_ts<256, 3>(budgets);
+        }
+    }
     switch (S) {
-        case 1: return sweep_fn_s<1>(budgets);
-        case 2: return sweep_fn_s<2>(budgets);
-        default: return sweep_fn_s<3>(budgets);
+        case 1: return sweep_fn_ts<128, 1>(budgets);
+        case 2: return sweep_fn_ts<128, 2>(budgets);
+        default: return sweep_fn_ts<128, 3>(budgets);
     }
 }
 static_assert(SWEEP_MAX_STEPS == 3, "instantiate sweep_kernel for every S up to SWEEP_MAX_STEPS");
+
+// 256-thread CTAs pay off only for the HBM-bound one-step pass over long rows (4 KB DRAM bursts per row
+// instead of 2 KB: 79 vs 74 G updates/s on config 4); the multi-step passes are faster with 128 (measured)
+bool sweep_wide(const bte_ctx* c, int S) {
+    if (c->sweep_threads != 0) return c->sweep_threads == 256;
+    return S == 1 && c->grid.n_phiy >= 4096;
+}
 
 int plan_sweep(bte_ctx* c) {
     int dev = 0, sms = 0;
@@ -201,10 +218,10 @@ int plan_sweep(bte_ctx* c) {
     const long long rows_alloc = c->grid.n_harm + 1 + 2 * GHOST;
     for (int S = 1; S <= SWEEP_MAX_STEPS; ++S) {
         c->sw_grid[S] = 0;
-        const SweepFn f = sweep_fn(S, c->has_budgets);
+        const SweepFn f = sweep_fn(S, c->has_budgets, sweep_wide(c, S));
         int occ = 0;
         cudaError_t e = cudaFuncSetAttribute(f.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f.smem);
-        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f.fn, FT, f.smem);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f.fn, f.T, f.smem);
         if (e != cudaSuccess)
             return fail(BTE_ECUDA, "sweep_kernel<S=%d> setup failed: %s (is this an sm_100a device?)", S,
                         cudaGetErrorString(e));
@@ -374,9 +391,9 @@ int launches_per_step(const bte_ctx* c) { return effective_variant(c) == VAR_SPL
 int launch_steps(bte_ctx* c, int S) {
     const int var = effective_variant(c);
     if (var == VAR_SWEEP) {
-        const SweepFn f = sweep_fn(S, c->has_budgets);
+        const SweepFn f = sweep_fn(S, c->has_budgets, sweep_wide(c, S));
         void* args[] = {&c->L};
-        CUDA_TRY(cudaLaunchKernel(f.fn, dim3(c->sw_grid[S]), dim3(FT), args, f.smem, c->stream));
+        CUDA_TRY(cudaLaunchKernel(f.fn, dim3(c->sw_grid[S]), dim3(f.T), args, f.smem, c->stream));
     } else if (var == VAR_FUSED) {
         fused_step_kernel<FT, FD><<<c->fgrid, FT, FCfg::smem_bytes, c->stream>>>(c->L, c->rows_per_chunk);
     } else {
@@ -411,9 +428,9 @@ int build_graph(bte_ctx* c, int64_t len, int S) {
             return e;
         };
         if (var == VAR_SWEEP) {
-            const SweepFn f = sweep_fn(S, c->has_budgets);
+            const SweepFn f = sweep_fn(S, c->has_budgets, sweep_wide(c, S));
             void* args[] = {&c->L};
-            CUDA_TRY(add(f.fn, dim3(c->sw_grid[S]), dim3(FT), f.smem, args));
+            CUDA_TRY(add(f.fn, dim3(c->sw_grid[S]), dim3(f.T), f.smem, args));
         } else if (var == VAR_FUSED) {
             void* args[] = {&c->L, &rpc};
             CUDA_TRY(add((void*)fused_step_kernel<FT, FD>, c->fgrid, dim3(FT), FCfg::smem_bytes, args));
@@ -554,7 +571,7 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
         if (params[s].n_steps_total > 0) c->budgets.push_back(params[s].n_steps_total);
     std::sort(c->budgets.begin(), c->budgets.end());
     c->budgets.erase(std::unique(c->budgets.begin(), c->budgets.end()), c->budgets.end());
-    c->sweep_steps = 0; c->sweep_ctas = 0; c->sm_count = 0; c->graph_S = 0;
+    c->sweep_steps = 0; c->sweep_ctas = 0; c->sm_count = 0; c->graph_S = 0; c->sweep_threads = 0;
     c->res_ctas_opt = 0; c->res_mode = -1; c->res_G = 0; c->res_Wc = 0; c->res_T = 0; c->res_smem = 0;
     for (int S = 0; S <= SWEEP_MAX_STEPS; ++S) c->sw_grid[S] = 0;
     c->steps_issued = 0; c->launches = 0;
@@ -754,6 +771,12 @@ int bte_set_option(bte_ctx* c, const char* key, int64_t value) {
         if (value < 0 || value > RES_MAX_CTAS) return fail(BTE_EINVAL, "resident_ctas must be in [0, %d]", RES_MAX_CTAS);
         c->res_ctas_opt = (int)value;
         return plan_resident(c);
+    }
+    if (!strcmp(key, "sweep_threads")) {   // threads per CTA of the sweep kernel: 128 or 256 (0 = automatic)
+        if (value != 0 && value != 128 && value != 256) return fail(BTE_EINVAL, "sweep_threads must be 0, 128 or 256");
+        c->sweep_threads = (int)value;
+        drop_graph(c);
+        return plan_sweep(c);
     }
     if (!strcmp(key, "sweep_steps")) {   // leap-frog steps fused per launch of the sweep kernel (0 = automatic)
         if (value < 0 || value > SWEEP_MAX_STEPS) return fail(BTE_EINVAL, "sweep_steps must be in [0, %d]", SWEEP_MAX_STEPS);

@@ -21,7 +21,7 @@ SWEEPS = ["sweep1", "sweep2", "sweep3"]
 ALL = ["split", "fused"] + SWEEPS + ["resident"]
 
 
-def gpu_solver(w, variant="auto", graph_steps=None, tile_rows=None, ctas=None, res_ctas=None):
+def gpu_solver(w, variant="auto", graph_steps=None, tile_rows=None, ctas=None, res_ctas=None, threads=None):
     from paper_1401_6047_b200 import Solver
     s = Solver(w.grid, w.params)
     s.set_option("variant", VARIANTS[variant][0])
@@ -34,13 +34,15 @@ def gpu_solver(w, variant="auto", graph_steps=None, tile_rows=None, ctas=None, r
         s.set_option("sweep_ctas", ctas)     # number of persistent CTAs of the sweep kernel
     if res_ctas is not None:
         s.set_option("resident_ctas", res_ctas)   # slabs of the resident kernel
+    if threads is not None:
+        s.set_option("sweep_threads", threads)    # 128 or 256 threads per CTA of the sweep kernel
     s.init_equilibrium()
     return s
 
 
 def check(w, n_steps, variant, systems=None, graph_steps=None, tile_rows=None, chunks=None, ctas=None,
-          res_ctas=None):
-    s = gpu_solver(w, variant, graph_steps, tile_rows, ctas, res_ctas)
+          res_ctas=None, threads=None):
+    s = gpu_solver(w, variant, graph_steps, tile_rows, ctas, res_ctas, threads)
     if chunks:                      # several bte_step calls must equal one
         for c in chunks:
             s.step(c)
@@ -90,6 +92,17 @@ def test_sweep_partition(ctas, variant):
     is not a multiple of S = 2, 3, so the trailing shorter launch is covered too."""
     w = W.small_case(N=21, M1=300, dt=0.004, n_steps=17, avg_start=3)
     check(w, 17, variant, ctas=ctas)
+
+
+@pytest.mark.parametrize("ctas", [1, 3, 11, 0])
+@pytest.mark.parametrize("variant", SWEEPS)
+def test_sweep_wide_ctas(ctas, variant):
+    """256-thread CTAs (strips of 254 / 250 / 246 columns): several strips with a ragged last one, segments cut
+    at arbitrary rows, single and batched."""
+    w = W.small_case(N=21, M1=600, dt=0.004, n_steps=10, avg_start=3)
+    check(w, 10, variant, ctas=ctas, threads=256)
+    wb = W.random_batch(n_batch=5, N=9, M1=300, dt=0.004, seed=78, periods=0.15)
+    check(wb, wb.n_steps + 2, variant, ctas=ctas, threads=256)
 
 
 @pytest.mark.parametrize("ctas", [1, 3, 9, 0])
