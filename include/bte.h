@@ -136,7 +136,7 @@ int bte_reconstruct_pdf(bte_ctx* ctx, int32_t system, int32_t grid_id, int32_t n
  *                  grid; 0 = automatic
  *   "sweep_steps"  S of variant 3: 1..3, 0 = automatic
  *   "sweep_ctas"   CTAs of the persistent sweep kernel, 0 = SMs x resident CTAs
- *   "sweep_threads" threads per CTA of the sweep kernel: 128 or 256, 0 = automatic
+ *   "sweep_threads" threads per CTA of the sweep kernel: 128, 256 or (one-step pass only) 512, 0 = automatic
  *   "graph_steps"  launches captured per CUDA graph for launch-bound grids; 0 = plain launches, -1 = auto
  *   "tile_rows"    rows per tile of variant 2 (0 = automatic)
  * Returns BTE_EINVAL for an unknown key or an unsupported value.                                        */

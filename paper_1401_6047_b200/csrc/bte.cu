@@ -182,12 +182,13 @@ struct SweepFn { void* fn; size_t smem; int W; int T; };
 template <int T, int S>
 SweepFn sweep_fn_ts(bool budgets) {
     using Cfg = SweepCfg<T, S>;
-    constexpr int MB = T == 128 ? SweepMinB<S>::v : (S == 1 ? 2 : 1);
+    constexpr int MB = T == 128 ? SweepMinB<S>::v : (S == 1 && T == 256 ? 2 : 1);
     return {budgets ? (void*)sweep_kernel<T, S, true, MB> : (void*)sweep_kernel<T, S, false, MB>,
             Cfg::smem_bytes, Cfg::W, T};
 }
 
-SweepFn sweep_fn(int S, bool budgets, bool wide) {
+SweepFn sweep_fn(int S, bool budgets, int wide) {
+    if (wide == 2 && S == 1) return sweep_fn_ts<512, 1>(budgets);
     if (wide) {
         switch (S) {
             case 1: return sweep_fn_ts<256, 1>(budgets);
@@ -203,11 +204,13 @@ SweepFn sweep_fn(int S, bool budgets, bool wide) {
 }
 static_assert(SWEEP_MAX_STEPS == 3, "instantiate sweep_kernel for every S up to SWEEP_MAX_STEPS");
 
-// 256-thread CTAs pay off only for the HBM-bound one-step pass over long rows (4 KB DRAM bursts per row
-// instead of 2 KB: 79 vs 74 G updates/s on config 4); the multi-step passes are faster with 128 (measured)
-bool sweep_wide(const bte_ctx* c, int S) {
-    if (c->sweep_threads != 0) return c->sweep_threads == 256;
-    return S == 1 && c->grid.n_phiy >= 4096;
+// Wider CTAs pay off only for the HBM-bound one-step pass over long rows (4 or 8 KB DRAM bursts per row instead
+// of 2 KB: 74 / 79 / 81 G updates/s on config 4 with 128 / 256 / 512 threads); the multi-step passes are faster
+// with 128 (measured).  Returns 0 / 1 / 2 for 128 / 256 / 512 threads.
+int sweep_wide(const bte_ctx* c, int S) {
+    if (c->sweep_threads != 0) return c->sweep_threads == 512 ? 2 : c->sweep_threads == 256 ? 1 : 0;
+    if (S != 1) return 0;
+    return c->grid.n_phiy >= 8192 ? 2 : c->grid.n_phiy >= 4096 ? 1 : 0;
 }
 
 int plan_sweep(bte_ctx* c) {
@@ -773,7 +776,8 @@ int bte_set_option(bte_ctx* c, const char* key, int64_t value) {
         return plan_resident(c);
     }
     if (!strcmp(key, "sweep_threads")) {   // threads per CTA of the sweep kernel: 128 or 256 (0 = automatic)
-        if (value != 0 && value != 128 && value != 256) return fail(BTE_EINVAL, "sweep_threads must be 0, 128 or 256");
+        if (value != 0 && value != 128 && value != 256 && value != 512)
+            return fail(BTE_EINVAL, "sweep_threads must be 0, 128, 256 or 512 (512: one-step pass only)");
         c->sweep_threads = (int)value;
         drop_graph(c);
         return plan_sweep(c);

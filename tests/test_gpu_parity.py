@@ -103,6 +103,9 @@ def test_sweep_wide_ctas(ctas, variant):
     check(w, 10, variant, ctas=ctas, threads=256)
     wb = W.random_batch(n_batch=5, N=9, M1=300, dt=0.004, seed=78, periods=0.15)
     check(wb, wb.n_steps + 2, variant, ctas=ctas, threads=256)
+    if variant == "sweep1":                       # 512-thread CTAs exist for the one-step pass only
+        w = W.small_case(N=21, M1=1100, dt=0.004, n_steps=10, avg_start=3)
+        check(w, 10, variant, ctas=ctas, threads=512)
 
 
 @pytest.mark.parametrize("ctas", [1, 3, 9, 0])
