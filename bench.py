@@ -343,6 +343,16 @@ def run_ours(args):
         "clocks": clocks,
         "check": {"norm": obs.norm, "v_dr": obs.v_dr, "step": obs.step, "e2e_step": obs2[0].step},
     }
+    if launches == 1 and args.steps > 1:
+        # resident kernel: the state never leaves the chip, HBM is not the roof.  Report against the fp64 pipe
+        # (148 SMs x 64 FMA lanes x 2 flop x 1.965 GHz; 26 FMA-class instructions per half-update).
+        line["roofline"] = {"bound": "alu", "achieved": 2 * fp64_rate / 1e12, "peak": 2 * fp64_peak / 1e12,
+                            "unit": "TFLOP/s", "frac": fp64_rate / fp64_peak, "traffic": None,
+                            "kernel": "resident_kernel", "steps_per_launch": steps_per_launch,
+                            "note": "whole time loop in one launch, state in shared memory; bounded by the serial "
+                                    "latency of a half-update plus one barrier (small lattices) or by the "
+                                    "shared-memory and fp64 pipes of the SM (DESIGN.md 5.2)",
+                            "peak_source": "derived: 148 SMs x 64 fp64 FMA/clk x 1.965 GHz (B200_PROFILING.md unit counts)"}
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(W.get(args.workload))
     print(json.dumps(line), flush=True)
