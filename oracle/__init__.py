@@ -6,7 +6,7 @@ this package.  It never imports paper_1401_6047_b200's CUDA binding and shares n
 
 
 def __getattr__(name):  # lazy, so that `python -m oracle.build` does not pre-import the wrapper
-    if name in ("OracleSim", "OracleObs", "max_threads"):
+    if name in ("OracleSim", "OracleObs", "max_threads", "pendulum_averages", "pendulum_trajectory"):
         from . import bte_oracle
         return getattr(bte_oracle, name)
     raise AttributeError(name)

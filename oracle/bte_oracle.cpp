@@ -15,7 +15,8 @@
  * Esaki-Tsu-type steady drift velocity, norm conservation, relaxation to f0, the B=0 mirror symmetry,
  * the field-reversal mirror, E=0 stationarity of f0 with order-2 convergence, order-2 convergence in
  * dt, the Tucker ac averages, a dense brute-force restatement on tiny grids, checkerboard independence
- * and affinity; the reconstruction of f (eq. 8) against eq. (13) at t = 0 and against a numpy contraction.  Absolute values of configs 1-4 have no closed form and the paper prints none:
+ * and affinity; the reconstruction of f (eq. 8) against eq. (13) at t = 0 and against a numpy contraction; the
+ * pendulum averages (eq. 44-46) against the T = 0 Esaki-Tsu and Tucker closed forms and the energy invariant.  Absolute values of configs 1-4 have no closed form and the paper prints none:
  * for those "parity unpinned" beyond the invariants listed above.
  *
  * Build: g++ -std=c++17 -O2 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).
@@ -291,6 +292,80 @@ void oracle_reconstruct_pdf(void* h, int32_t grid, int32_t K, double* f) {
                 acc += a[idx(s, n, m)] * std::cos(n * x) + b[idx(s, n, m)] * std::sin(n * x);
             f[(size_t)i * s->M1 + m] = acc;
         }
+    }
+}
+
+/* ---- the zero-temperature limit, eq. (44)-(46) ---------------------
+ * A single electron starts at (phi_x, phi_y) = (0, 0) (f0 -> delta function, L217) at time t0 and follows
+ *     d phi_x / dt = E(t) + B phi_y            (44)        E(t) = E_dc + E_omega cos(omega t)   (L99)
+ *     d phi_y / dt = -B sin(phi_x)             (45)
+ * Its velocity along x is sin(phi_x) (dispersion (3) in the units of (4)).  Dissipation re-enters through the
+ * exponential memory (46): v_dr(t) = int_{-inf}^{t} sin phi_x(t; t0) e^{-(t - t0)} dt0.  Averaged over one ac period
+ * (t0 -> start phase, s = t - t0):
+ *     <v_dr>          = (1/T) int_0^T dt0 int_0^inf ds e^{-s} sin phi_x(t0 + s; t0)
+ *     <v_dr cos wt>   = (1/T) int_0^T dt0 int_0^inf ds e^{-s} sin phi_x(t0 + s; t0) cos(w (t0 + s))     (17), I1/I0 -> 1
+ * The paper gives no discretisation ("can be trivially solved numerically", L235); reading taken (C20):
+ * classical RK4 with step h for (44)-(45), composite Simpson on the RK4 nodes s_k = k h, k = 0..n_rk (n_rk even,
+ * memory cut at n_rk h), rectangle rule over n_phase equidistant start phases t0_j = j T / n_phase (periodic
+ * integrand).  Without an ac field (E_omega = 0 or omega = 0) one start phase, t0 = 0.
+ * out[0..2] = <v_dr>, <v_dr cos wt>, <v_dr sin wt>.                                                             */
+static void pendulum_rhs(double Edc, double Ew, double w, double B, double t, double px, double py, double* dx,
+                         double* dy) {
+    *dx = (Edc + Ew * std::cos(w * t)) + B * py;
+    *dy = -B * std::sin(px);
+}
+
+void oracle_pendulum_averages(double Edc, double Ew, double w, double B, int32_t n_phase, double h, int32_t n_rk,
+                              double* out) {
+    const double PI = 3.14159265358979323846;
+    const bool ac = (Ew != 0.0) && (w != 0.0);
+    const int P = ac ? n_phase : 1;
+    const double T = ac ? 2.0 * PI / w : 0.0;
+    double sum0 = 0.0, sumc = 0.0, sums = 0.0;
+    for (int j = 0; j < P; ++j) {
+        const double t0 = ac ? T * j / P : 0.0;
+        double px = 0.0, py = 0.0, I0 = 0.0, Ic = 0.0, Is = 0.0;
+        for (int k = 0; k <= n_rk; ++k) {
+            const double s = k * h, t = t0 + s;
+            const double wgt = (k == 0 || k == n_rk) ? 1.0 : ((k & 1) ? 4.0 : 2.0);
+            const double g = std::exp(-s) * std::sin(px);
+            I0 += wgt * g;
+            Ic += wgt * g * std::cos(w * t);
+            Is += wgt * g * std::sin(w * t);
+            if (k == n_rk) break;
+            double k1x, k1y, k2x, k2y, k3x, k3y, k4x, k4y;
+            pendulum_rhs(Edc, Ew, w, B, t, px, py, &k1x, &k1y);
+            pendulum_rhs(Edc, Ew, w, B, t + 0.5 * h, px + 0.5 * h * k1x, py + 0.5 * h * k1y, &k2x, &k2y);
+            pendulum_rhs(Edc, Ew, w, B, t + 0.5 * h, px + 0.5 * h * k2x, py + 0.5 * h * k2y, &k3x, &k3y);
+            pendulum_rhs(Edc, Ew, w, B, t + h, px + h * k3x, py + h * k3y, &k4x, &k4y);
+            px += (h / 6.0) * (k1x + 2.0 * k2x + 2.0 * k3x + k4x);
+            py += (h / 6.0) * (k1y + 2.0 * k2y + 2.0 * k3y + k4y);
+        }
+        sum0 += I0 * (h / 3.0);
+        sumc += Ic * (h / 3.0);
+        sums += Is * (h / 3.0);
+    }
+    out[0] = sum0 / P;
+    out[1] = sumc / P;
+    out[2] = sums / P;
+}
+
+/* Test hook: the trajectory itself, n_rk + 1 nodes from (0, 0) at t0 (for the energy-invariant pin). */
+void oracle_pendulum_trajectory(double Edc, double Ew, double w, double B, double t0, double h, int32_t n_rk,
+                                double* px_out, double* py_out) {
+    double px = 0.0, py = 0.0;
+    for (int k = 0; k <= n_rk; ++k) {
+        px_out[k] = px;
+        py_out[k] = py;
+        if (k == n_rk) break;
+        const double t = t0 + k * h;
+        double k1x, k1y, k2x, k2y, k3x, k3y, k4x, k4y;
+        pendulum_rhs(Edc, Ew, w, B, t, px, py, &k1x, &k1y);
+        pendulum_rhs(Edc, Ew, w, B, t + 0.5 * h, px + 0.5 * h * k1x, py + 0.5 * h * k1y, &k2x, &k2y);
+        pendulum_rhs(Edc, Ew, w, B, t + 0.5 * h, px + 0.5 * h * k2x, py + 0.5 * h * k2y, &k3x, &k3y);
+        pendulum_rhs(Edc, Ew, w, B, t + h, px + h * k3x, py + h * k3y, &k4x, &k4y);
+        px += (h / 6.0) * (k1x + 2.0 * k2x + 2.0 * k3x + k4x);
+        py += (h / 6.0) * (k1y + 2.0 * k2y + 2.0 * k3y + k4y);
     }
 }
 

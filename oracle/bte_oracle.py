@@ -55,6 +55,8 @@ def _load():
         lib.oracle_get_equilibrium.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         lib.oracle_apply_T.argtypes = [C.c_void_p, C.c_int32, C.c_double, C.c_double, C.c_double]
         lib.oracle_reconstruct_pdf.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
+        lib.oracle_pendulum_averages.argtypes = [C.c_double] * 4 + [C.c_int32, C.c_double, C.c_int32, C.c_void_p]
+        lib.oracle_pendulum_trajectory.argtypes = [C.c_double] * 6 + [C.c_int32, C.c_void_p, C.c_void_p]
         lib.oracle_max_threads.restype = C.c_int32
         _lib = lib
     return _lib
@@ -62,6 +64,19 @@ def _load():
 
 def max_threads() -> int:
     return int(_load().oracle_max_threads())
+
+
+def pendulum_averages(E_dc, E_omega, omega, B, n_phase, h, n_rk):
+    """(<v_dr>, <v_dr cos wt>, <v_dr sin wt>) of the zero-temperature pendulum model, eq. (44)-(46)."""
+    out = np.zeros(3)
+    _load().oracle_pendulum_averages(E_dc, E_omega, omega, B, n_phase, h, n_rk, out.ctypes.data)
+    return tuple(float(x) for x in out)
+
+
+def pendulum_trajectory(E_dc, E_omega, omega, B, t0, h, n_rk):
+    px, py = np.zeros(n_rk + 1), np.zeros(n_rk + 1)
+    _load().oracle_pendulum_trajectory(E_dc, E_omega, omega, B, t0, h, n_rk, px.ctypes.data, py.ctypes.data)
+    return px, py
 
 
 class OracleSim:

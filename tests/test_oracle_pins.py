@@ -486,3 +486,41 @@ def test_pdf_reconstruction_is_the_fourier_sum_of_any_state():
     want = np.einsum("in,nm->im", np.cos(np.outer(x, n)), a) + np.einsum("in,nm->im", np.sin(np.outer(x, n)), b)
     assert np.abs(f - want).max() <= 1e-13
     assert abs(f[K // 2, 3] - a[:, 3].sum()) <= 1e-13            # phi_x = 0: cos = 1, sin = 0
+
+
+# ---------------------------------------------------------------------------------------------------
+# NEXT-2: zero-temperature pendulum model, eq. (44)-(46)
+# ---------------------------------------------------------------------------------------------------
+def test_pendulum_dc_B0_is_esaki_tsu_at_T0():
+    """B = 0, dc field: phi_x = E s, so <v_dr> = int_0^S e^{-s} sin(E s) ds in closed form (S -> inf: E/(1+E^2))."""
+    from oracle import pendulum_averages
+    for E in (0.3, 1.0, 2.5):
+        S, h = 40.0, 0.005
+        v, vc, vs = pendulum_averages(E, 0.0, 0.0, 0.0, 1, h, int(round(S / h)))
+        want = (E - math.exp(-S) * (E * math.cos(E * S) + math.sin(E * S))) / (1 + E * E)
+        assert abs(v - want) < 1e-10                  # Simpson: O(h^4)
+        assert abs(want - E / (1 + E * E)) < 1e-15
+
+
+def test_pendulum_ac_B0_is_tucker_at_T0():
+    """B = 0 with an ac field: the Tucker sums (eq. 42-43) with I1/I0 -> 1 (mu -> infinity)."""
+    from oracle import pendulum_averages
+    from parity_util import tucker_averages
+    E_dc, E_w, w = 2.0, 0.5, 1.5
+    v, vc, vs = pendulum_averages(E_dc, E_w, w, 0.0, 64, 0.004, 10000)
+    r = float(special.ive(1, 1e6) / special.ive(0, 1e6))       # -> 1
+    v_ref, vc_ref, _ = tucker_averages(1e6, E_dc, E_w, w)
+    assert abs(v - v_ref / r) < 1e-9 and abs(vc - vc_ref / r) < 1e-9
+
+
+def test_pendulum_energy_invariant_and_phase_count():
+    """Constant E: (E + B phi_y)^2 / 2 - B^2 cos(phi_x) is conserved by (44)-(45) (RK4: to O(h^4)); and the phase
+    average is converged (64 vs 128 start phases agree: periodic rectangle rule)."""
+    from oracle import pendulum_averages, pendulum_trajectory
+    E, B, h = 3.0, 2.0, 0.002
+    px, py = pendulum_trajectory(E, 0.0, 0.0, B, 0.0, h, 10000)
+    inv = 0.5 * (E + B * py) ** 2 - B * B * np.cos(px)
+    assert np.abs(inv - inv[0]).max() < 1e-9 * abs(inv[0])
+    a = pendulum_averages(6.0, 0.1, 4.0, 4.0, 64, 0.004, 7500)
+    b = pendulum_averages(6.0, 0.1, 4.0, 4.0, 128, 0.004, 7500)
+    assert max(abs(x - y) for x, y in zip(a, b)) < 1e-10
