@@ -124,6 +124,20 @@ int bte_set_state(bte_ctx* ctx, int32_t system, int32_t grid_id, const double* a
  * Reads the step counter's buffer flag (synchronises the stream once), then runs asynchronously on the stream. */
 int bte_reconstruct_pdf(bte_ctx* ctx, int32_t system, int32_t grid_id, int32_t n_phix, double* f /* device */);
 
+/* The zero-temperature limit of the model, eq. (44)-(46) (L229-240): one electron starts at (phi_x, phi_y) = (0, 0) and
+ * follows d phi_x/dt = E(t) + B phi_y, d phi_y/dt = -B sin(phi_x); its velocity sin(phi_x) enters the drift velocity
+ * through the exponential memory (46).  Returns, per parameter set, the averages over one ac period
+ *   v_mean = <v_dr>, v_cos = <v_dr cos wt>, v_sin = <v_dr sin wt>      (absorption of eq. (17) at T -> 0: A = 2 v_cos).
+ * Discretisation (C20): classical RK4 with step h, composite Simpson on the n_rk + 1 RK4 nodes (n_rk even;
+ * the memory is cut at n_rk h), rectangle rule over n_phase start phases (1 is used when E_omega or omega is 0).
+ *   params, out : HOST arrays of n entries;  workspace : DEVICE, caller-owned, >= bte_pendulum_workspace_bytes(n).
+ * Independent of any ctx.  Synchronises the stream before returning.                                          */
+typedef struct { double E_dc, E_omega, omega, B; } bte_pendulum_params;
+typedef struct { double v_mean, v_cos, v_sin; } bte_pendulum_out;
+size_t bte_pendulum_workspace_bytes(int32_t n);
+int bte_pendulum_averages(const bte_pendulum_params* params, int32_t n, int32_t n_phase, double h, int32_t n_rk,
+                          void* workspace /* device */, size_t bytes, void* cuda_stream, bte_pendulum_out* out);
+
 /* Tuning / variant selection, before or between bte_step calls.  Keys:
  *   "variant"      0 = automatic (default), 1 = two half-update kernels per step (96 B/point/step),
  *                  2 = fused whole+fractional kernel on a 2-D tile grid (64 B/point/step),

@@ -19,7 +19,8 @@ LIB_PATH = os.path.join(_HERE, "libbte_b200.so")
 BTE_OK, BTE_EINVAL, BTE_EUNSTABLE, BTE_ENOMEM, BTE_ECUDA = 0, -1, -2, -3, -4
 
 EXPORTS = ("bte_workspace_bytes", "bte_create", "bte_init_equilibrium", "bte_step", "bte_observables",
-           "bte_destroy", "bte_get_state", "bte_set_state", "bte_reconstruct_pdf", "bte_set_option", "bte_launch_count",
+           "bte_destroy", "bte_get_state", "bte_set_state", "bte_reconstruct_pdf", "bte_pendulum_workspace_bytes",
+           "bte_pendulum_averages", "bte_set_option", "bte_launch_count",
            "bte_last_error")
 
 
@@ -88,6 +89,11 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.bte_set_state.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
     lib.bte_reconstruct_pdf.restype = C.c_int
     lib.bte_reconstruct_pdf.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p]
+    lib.bte_pendulum_workspace_bytes.restype = C.c_size_t
+    lib.bte_pendulum_workspace_bytes.argtypes = [C.c_int32]
+    lib.bte_pendulum_averages.restype = C.c_int
+    lib.bte_pendulum_averages.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_int32, C.c_void_p,
+                                          C.c_size_t, C.c_void_p, C.c_void_p]
     lib.bte_set_option.restype = C.c_int
     lib.bte_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_int64]
     lib.bte_launch_count.restype = C.c_int
@@ -113,6 +119,25 @@ def make_params(ps: Sequence) -> C.Array:
         arr[i] = bte_params(p.E_dc, p.E_omega, p.omega, p.B, p.mu, p.alpha, p.phiy_min, p.phiy_max,
                             p.kappa_scale, int(p.n_steps_total), int(p.avg_start_step))
     return arr
+
+
+def pendulum_averages(param_sets, n_phase: int = 64, h: float = 0.004, n_rk: int = 7500, device: str = "cuda:0"):
+    """Zero-temperature pendulum model, eq. (44)-(46): param_sets = [(E_dc, E_omega, omega, B), ...]; returns a list
+    of (v_mean, v_cos, v_sin).  Argument marshalling only: the integration runs in the library's kernel."""
+    import torch
+    lib = load_library()
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_1401_6047_b200 needs a CUDA device (no CPU fallback)")
+    n = len(param_sets)
+    arr = (C.c_double * (4 * n))(*[float(x) for ps in param_sets for x in ps])
+    out = (C.c_double * (3 * n))()
+    nbytes = int(lib.bte_pendulum_workspace_bytes(n))
+    with torch.cuda.device(device):
+        ws = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=device)
+        stream = torch.cuda.current_stream().cuda_stream
+        _check(lib.bte_pendulum_averages(arr, n, n_phase, h, n_rk, C.c_void_p(ws.data_ptr()), ws.numel(),
+                                         C.c_void_p(stream), out))
+    return [(out[3 * i], out[3 * i + 1], out[3 * i + 2]) for i in range(n)]
 
 
 def workspace_bytes(n_harm: int, n_phiy: int, n_batch: int, dt: float) -> int:

@@ -3,6 +3,7 @@
 #include "../../include/bte.h"
 #include "bte_sweep.cuh"
 #include "bte_resident.cuh"
+#include "bte_pendulum.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -742,6 +743,33 @@ int bte_reconstruct_pdf(bte_ctx* c, int32_t system, int32_t grid_id, int32_t n_p
     pdf_kernel<KT><<<g, 128, 2 * (size_t)n_phix * sizeof(double), c->stream>>>(z, f, rows, M1, pitch, n_phix);
     CUDA_TRY(cudaGetLastError());
     c->launches += 1;
+    return BTE_OK;
+}
+
+size_t bte_pendulum_workspace_bytes(int32_t n) {
+    return n < 1 ? 0 : (size_t)n * (sizeof(PendulumParams) + sizeof(PendulumOut));
+}
+
+int bte_pendulum_averages(const bte_pendulum_params* params, int32_t n, int32_t n_phase, double h, int32_t n_rk,
+                          void* workspace, size_t bytes, void* cuda_stream, bte_pendulum_out* out) {
+    static_assert(sizeof(bte_pendulum_params) == sizeof(PendulumParams) && sizeof(bte_pendulum_out) == sizeof(PendulumOut),
+                  "ABI structs mirror the device structs");
+    if (!params || !out || !workspace) return fail(BTE_EINVAL, "bte_pendulum_averages: NULL argument");
+    if (n < 1 || n > 65535 || n_phase < 1 || n_rk < 2 || (n_rk & 1) || !(h > 0.0) || !std::isfinite(h))
+        return fail(BTE_EINVAL, "bte_pendulum_averages: need 1 <= n <= 65535, n_phase >= 1, even n_rk >= 2, h > 0");
+    for (int i = 0; i < n; ++i)
+        if (!std::isfinite(params[i].E_dc) || !std::isfinite(params[i].E_omega) || !std::isfinite(params[i].omega) ||
+            !std::isfinite(params[i].B))
+            return fail(BTE_EINVAL, "bte_pendulum_averages: parameter set %d is not finite", i);
+    if (bytes < bte_pendulum_workspace_bytes(n)) return fail(BTE_ENOMEM, "bte_pendulum_averages: workspace too small");
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    PendulumParams* dp = (PendulumParams*)workspace;
+    PendulumOut* dout = (PendulumOut*)((char*)workspace + (size_t)n * sizeof(PendulumParams));
+    CUDA_TRY(cudaMemcpyAsync(dp, params, (size_t)n * sizeof(PendulumParams), cudaMemcpyHostToDevice, stream));
+    pendulum_kernel<<<n, 128, 0, stream>>>(dp, dout, n_phase, h, n_rk);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaMemcpyAsync(out, dout, (size_t)n * sizeof(PendulumOut), cudaMemcpyDeviceToHost, stream));
+    CUDA_TRY(cudaStreamSynchronize(stream));
     return BTE_OK;
 }
 
