@@ -157,9 +157,18 @@ def cpu_baseline(w, target_seconds=12.0):
     t0 = time.perf_counter()
     sim.step(n)
     el = time.perf_counter() - t0
+    # the same oracle on ONE thread (the paper's own CPU figure is single-threaded)
+    sim1 = OracleSim(w.grid.n_harm, w.grid.n_phiy, w.grid.dt, w.params[0], threads=1)
+    sim1.init_equilibrium()
+    n1 = int(max(1, min(n, (target_seconds / 3.0) / (one * threads))))
+    t0 = time.perf_counter()
+    sim1.step(n1)
+    el1 = time.perf_counter() - t0
     return {"value": pts * n / el, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "value_1_thread": pts * n1 / el1,
             "sample": f"oracle/bte_oracle.cpp, steps 2..{n + 1} of {w.name} system 0 "
-                      f"({pts} points/step), {threads} OpenMP threads, {el:.1f} s"}
+                      f"({pts} points/step), {threads} OpenMP threads, {el:.1f} s; then {n1} step(s) on 1 thread, "
+                      f"{el1:.1f} s"}
 
 
 # ---------------------------------------------------------------------------------------------------
