@@ -45,9 +45,11 @@ struct Sim {
     std::vector<double> a0;             /* a_n^(0)(m), eq. (15)                                          */
     std::vector<double> ha, hb, fa, fb; /* whole grid z_h and fractional grid z_f, eq. (39)-(41)         */
     std::vector<double> sa, sb;         /* snapshot used only by the start-up step                       */
+    std::vector<float> cf, gf;          /* precision 2: c_n and g_m = exp(-mu phi^2/2) rounded to fp32   */
     int64_t step;
     double norm, v_dr, sum_v, sum_c, sum_s, window;
     int threads;
+    int precision;          /* 0: fp64 (default); 1: state stored as fp32, arithmetic fp64; 2: fp32 throughout (NEXT-4) */
 };
 
 inline size_t idx(const Sim* s, int n, int m) { return (size_t)n * (size_t)s->M1 + (size_t)m; }
@@ -106,8 +108,60 @@ void apply_T(const Sim* s, double delta, double* Xa, double* Xb, const double* S
             const double det = nu * nu + mu_b * mu_b;
             Xa[i] = (g * nu - h * mu_b) / det;
             Xb[i] = (n >= 1) ? (g * mu_b + h * nu) / det : 0.0;
+            if (s->precision == 1) { /* the state lives in fp32 storage: every new value is rounded once */
+                Xa[i] = (double)(float)Xa[i];
+                Xb[i] = (double)(float)Xb[i];
+            }
         }
     }
+}
+
+/* The same operator T with every quantity and every operation in fp32, "all code used float data type"
+ * (PAPER.md:L311), SURVEY 8(f) NEXT-4.  The arrays hold values that are exactly representable in fp32.  Scalars that
+ * do not depend on the lattice point (E(t), kappa, nu, xi) are formed in fp64 and rounded once; c_n and the Gaussian
+ * factor g_m are rounded to fp32 and a^(0) delta is formed as c_n (g_m delta).  Operation order as written, one
+ * rounding per operation (-ffp-contract=off), IEEE division.                                                      */
+void apply_T_f32(const Sim* s, double delta_d, double* Xa, double* Xb, const double* Sa, const double* Sb, double ta,
+                 double tb, const std::vector<float>& cf, const std::vector<float>& gf) {
+    const int N = s->N, M1 = s->M1;
+    const float delta = (float)delta_d;
+    const float kappa = (float)(s->kappa_scale * s->B * delta_d / (4.0 * s->dphi));
+    const float nu = (float)(1.0 + delta_d / 2.0);
+    const float xi = (float)(1.0 - delta_d / 2.0);
+    const float Ea = (float)field_E(s, ta);
+    const float Eb = (float)field_E(s, tb);
+    const float Bf = (float)s->B;
+#pragma omp parallel for schedule(static) num_threads(s->threads)
+    for (int n = 0; n <= N; ++n) {
+        const float nf = (float)n;
+        for (int m = 0; m < M1; ++m) {
+            const float ph = (float)s->phi[m];
+            const float beta_a = Ea + Bf * ph;
+            const float beta_b = Eb + Bf * ph;
+            const float mu_a = nf * beta_a * delta / 2.0f;
+            const float mu_b = nf * beta_b * delta / 2.0f;
+            const float chi = (n == 1) ? 2.0f : 1.0f;
+            const float Bt = kappa * ((float)rd_b(s, Sb, n + 1, m + 1) - (float)rd_b(s, Sb, n + 1, m - 1) -
+                                      (float)rd_b(s, Sb, n - 1, m + 1) + (float)rd_b(s, Sb, n - 1, m - 1));
+            const float At = kappa * (chi * ((float)rd_a(s, Sa, n - 1, m + 1) - (float)rd_a(s, Sa, n - 1, m - 1)) -
+                                      (float)rd_a(s, Sa, n + 1, m + 1) + (float)rd_a(s, Sa, n + 1, m - 1));
+            const size_t i = idx(s, n, m);
+            const float a = (float)Xa[i];
+            const float b = (float)Xb[i];
+            const float src = cf[n] * (gf[m] * delta);
+            const float g = a * xi - b * mu_a + Bt + src;
+            const float h = b * xi + a * mu_a + At;
+            const float det = nu * nu + mu_b * mu_b;
+            Xa[i] = (double)((g * nu - h * mu_b) / det);
+            Xb[i] = (n >= 1) ? (double)((g * mu_b + h * nu) / det) : 0.0;
+        }
+    }
+}
+
+void run_T(const Sim* s, double delta, double* Xa, double* Xb, const double* Sa, const double* Sb, double ta,
+           double tb) {
+    if (s->precision == 2) apply_T_f32(s, delta, Xa, Xb, Sa, Sb, ta, tb, s->cf, s->gf);
+    else apply_T(s, delta, Xa, Xb, Sa, Sb, ta, tb);
 }
 
 /* phi_y lattice (reading C8) and equilibrium coefficients, eq. (15)-(16) with sigma(0) = 1/2,
@@ -122,6 +176,8 @@ void fill_equilibrium(Sim* s) {
     const double i0 = std::cyl_bessel_i(0.0, s->mu);
     const double pref = std::sqrt(s->mu / (2.0 * PI * s->alpha));
     s->a0.assign((size_t)(N + 1) * M1, 0.0);
+    s->cf.assign(N + 1, 0.0f);
+    s->gf.assign(M1, 0.0f);
     for (int n = 0; n <= N; ++n) {
         const double r = std::cyl_bessel_i((double)n, s->mu) / i0;
         const double c = (n == 0) ? (1.0 / (2.0 * PI)) * pref : (r / PI) * pref;
@@ -129,7 +185,9 @@ void fill_equilibrium(Sim* s) {
             double gm = std::exp(-s->mu * s->phi[m] * s->phi[m] / 2.0);
             if (gm < 1e-300) gm = 0.0;
             s->a0[idx(s, n, m)] = c * gm;
+            s->gf[m] = (float)gm;
         }
+        s->cf[n] = (float)c;
     }
 }
 
@@ -168,6 +226,7 @@ void* oracle_create(int32_t n_harm, int32_t n_phiy, double dt, const oracle_para
     s->kappa_scale = p->kappa_scale;
     s->n_steps_total = p->n_steps_total; s->avg_start_step = p->avg_start_step;
     s->threads = threads > 0 ? threads : 1;
+    s->precision = 0;
     fill_equilibrium(s);
     const size_t P = (size_t)(s->N + 1) * s->M1;
     s->ha.assign(P, 0.0); s->hb.assign(P, 0.0); s->fa.assign(P, 0.0); s->fb.assign(P, 0.0);
@@ -177,15 +236,24 @@ void* oracle_create(int32_t n_harm, int32_t n_phiy, double dt, const oracle_para
 
 void oracle_destroy(void* h) { delete (Sim*)h; }
 
+/* NEXT-4: 0 = fp64 (default), 1 = state stored in fp32 / arithmetic fp64, 2 = fp32 throughout.  Call before
+ * oracle_init_equilibrium.                                                                                    */
+void oracle_set_precision(void* h, int32_t precision) { ((Sim*)h)->precision = precision; }
+
 /* Initial condition a = a^(0), b = 0 and start-up of the fractional grid: z^{1/2} by
  * (38) with time step dt/2 (reading C6: delta = dt/2 everywhere, stencil from z^0,
  * field times 0 and dt/2).                                                                             */
 void oracle_init_equilibrium(void* h) {
     Sim* s = (Sim*)h;
     s->ha = s->a0;
+    if (s->precision == 1)
+        for (double& x : s->ha) x = (double)(float)x;
+    if (s->precision == 2)
+        for (int n = 0; n <= s->N; ++n)
+            for (int m = 0; m < s->M1; ++m) s->ha[idx(s, n, m)] = (double)(s->cf[n] * s->gf[m]);
     std::fill(s->hb.begin(), s->hb.end(), 0.0);
     s->fa = s->ha; s->fb = s->hb;
-    apply_T(s, s->dt / 2.0, s->fa.data(), s->fb.data(), s->ha.data(), s->hb.data(), 0.0, s->dt / 2.0);
+    run_T(s, s->dt / 2.0, s->fa.data(), s->fb.data(), s->ha.data(), s->hb.data(), 0.0, s->dt / 2.0);
     s->step = 0; s->sum_v = s->sum_c = s->sum_s = s->window = 0.0;
     reduce_observables(s);
 }
@@ -195,7 +263,7 @@ void oracle_init_equilibrium(void* h) {
 void oracle_startup_from_whole(void* h) {
     Sim* s = (Sim*)h;
     s->fa = s->ha; s->fb = s->hb;
-    apply_T(s, s->dt / 2.0, s->fa.data(), s->fb.data(), s->ha.data(), s->hb.data(), 0.0, s->dt / 2.0);
+    run_T(s, s->dt / 2.0, s->fa.data(), s->fb.data(), s->ha.data(), s->hb.data(), 0.0, s->dt / 2.0);
     s->step = 0; s->sum_v = s->sum_c = s->sum_s = s->window = 0.0;
     reduce_observables(s);
 }
@@ -214,9 +282,9 @@ void oracle_step(void* h, int64_t n_steps, double* v_trace, double* norm_trace) 
             continue;
         }
         const double k = (double)s->step;
-        apply_T(s, s->dt, s->ha.data(), s->hb.data(), s->fa.data(), s->fb.data(), k * s->dt,
+        run_T(s, s->dt, s->ha.data(), s->hb.data(), s->fa.data(), s->fb.data(), k * s->dt,
                 (k + 1.0) * s->dt);
-        apply_T(s, s->dt, s->fa.data(), s->fb.data(), s->ha.data(), s->hb.data(), (k + 0.5) * s->dt,
+        run_T(s, s->dt, s->fa.data(), s->fb.data(), s->ha.data(), s->hb.data(), (k + 0.5) * s->dt,
                 (k + 1.5) * s->dt);
         s->step += 1;
         const double t = (double)s->step * s->dt;
@@ -270,9 +338,9 @@ void oracle_get_equilibrium(void* h, double* phi, double* a0) {
 void oracle_apply_T(void* h, int32_t target, double delta, double ta, double tb) {
     Sim* s = (Sim*)h;
     if (target == 0)
-        apply_T(s, delta, s->ha.data(), s->hb.data(), s->fa.data(), s->fb.data(), ta, tb);
+        run_T(s, delta, s->ha.data(), s->hb.data(), s->fa.data(), s->fb.data(), ta, tb);
     else
-        apply_T(s, delta, s->fa.data(), s->fb.data(), s->ha.data(), s->hb.data(), ta, tb);
+        run_T(s, delta, s->fa.data(), s->fb.data(), s->ha.data(), s->hb.data(), ta, tb);
 }
 
 /* The distribution function itself, eq. (8): f(phi_x, phi_y) = sum_n a_n cos(n phi_x) + b_n sin(n phi_x), written

@@ -46,6 +46,7 @@ def _load():
         lib.oracle_create.restype = C.c_void_p
         lib.oracle_create.argtypes = [C.c_int32, C.c_int32, C.c_double, C.POINTER(_Params), C.c_int32]
         lib.oracle_destroy.argtypes = [C.c_void_p]
+        lib.oracle_set_precision.argtypes = [C.c_void_p, C.c_int32]
         lib.oracle_init_equilibrium.argtypes = [C.c_void_p]
         lib.oracle_startup_from_whole.argtypes = [C.c_void_p]
         lib.oracle_step.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
@@ -82,7 +83,8 @@ def pendulum_trajectory(E_dc, E_omega, omega, B, t0, h, n_rk):
 class OracleSim:
     """One system.  `params` is any object with the fields of workloads.Params."""
 
-    def __init__(self, n_harm: int, n_phiy: int, dt: float, params, threads: int = 1):
+    def __init__(self, n_harm: int, n_phiy: int, dt: float, params, threads: int = 1, precision: int = 0):
+        """precision: 0 = fp64, 1 = state stored in fp32 / fp64 arithmetic, 2 = fp32 throughout (NEXT-4)."""
         lib = _load()
         p = _Params(params.E_dc, params.E_omega, params.omega, params.B, params.mu, params.alpha,
                     params.phiy_min, params.phiy_max, params.kappa_scale,
@@ -90,6 +92,7 @@ class OracleSim:
         self._h = lib.oracle_create(n_harm, n_phiy, dt, C.byref(p), threads)
         if not self._h:
             raise ValueError("oracle_create: invalid arguments")
+        lib.oracle_set_precision(self._h, precision)
         self.N, self.M1, self.dt, self.threads = n_harm, n_phiy, dt, threads
         self.shape = (n_harm + 1, n_phiy)
 

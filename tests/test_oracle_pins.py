@@ -524,3 +524,41 @@ def test_pendulum_energy_invariant_and_phase_count():
     a = pendulum_averages(6.0, 0.1, 4.0, 4.0, 64, 0.004, 7500)
     b = pendulum_averages(6.0, 0.1, 4.0, 4.0, 128, 0.004, 7500)
     assert max(abs(x - y) for x, y in zip(a, b)) < 1e-10
+
+
+# ---------------------------------------------------------------------------------------------------
+# NEXT-4: fp32 storage / fp32 arithmetic (the paper's precision, L311) and its time-step floor (L328)
+# ---------------------------------------------------------------------------------------------------
+def _run_prec(precision, dt, t_end, N=8, M1=81):
+    from paper_1401_6047_b200 import workloads as W
+    w = W.small_case(N=N, M1=M1, dt=dt, E_dc=2.0, E_omega=0.0, omega=0.0, B=1.0, mu=2.0, phiy_max=6.0)
+    sim = OracleSim(N, M1, dt, w.params[0], threads=2, precision=precision)
+    sim.init_equilibrium()
+    sim.step(int(round(t_end / dt)))
+    return sim
+
+
+def test_fp32_modes_stay_close_to_fp64_and_hold_fp32_values():
+    ref = _run_prec(0, 0.004, 0.4)
+    ra, rb = ref.get_state(0)
+    scale = max(np.abs(ra).max(), np.abs(rb).max())
+    for prec in (1, 2):
+        s = _run_prec(prec, 0.004, 0.4)
+        a, b = s.get_state(0)
+        assert np.array_equal(a, a.astype(np.float32).astype(np.float64))      # exactly representable in fp32
+        assert np.array_equal(b, b.astype(np.float32).astype(np.float64))
+        err = max(np.abs(a - ra).max(), np.abs(b - rb).max()) / scale
+        assert 0 < err < 1e-5, (prec, err)                                      # O(eps32 / dt), not zero
+        assert abs(s.observables().v_dr - ref.observables().v_dr) < 1e-5
+
+
+def test_fp32_norm_drift_grows_as_dt_shrinks():
+    """in float the norm of f drifts away from 1 when the time step gets small (the paper saw it
+    'diverge' for dt <= 1e-5).  Every step adds a rounding error O(eps32) that the relaxation removes at rate dt, so
+    the drift at fixed t scales like eps32 / dt; in fp64 it is invisible."""
+    drift = {dt: abs(_run_prec(2, dt, 0.5).observables().norm - 1.0) for dt in (1e-2, 1e-3, 1e-4)}
+    assert drift[1e-3] > 3 * drift[1e-2] and drift[1e-4] > 3 * drift[1e-3], drift
+    assert drift[1e-4] > 3e-5
+    assert abs(_run_prec(0, 1e-4, 0.5).observables().norm - 1.0) < 1e-12
+    d1 = abs(_run_prec(1, 1e-4, 0.5).observables().norm - 1.0)
+    assert 1e-8 < d1 < drift[1e-4] / 10      # storage rounding alone: unbiased, a random walk -- far smaller
