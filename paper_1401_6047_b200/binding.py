@@ -32,7 +32,7 @@ class BteError(RuntimeError):
 
 class bte_grid(C.Structure):
     _fields_ = [("n_harm", C.c_int32), ("n_phiy", C.c_int32), ("n_batch", C.c_int32),
-                ("reserved", C.c_int32), ("dt", C.c_double)]
+                ("precision", C.c_int32), ("dt", C.c_double)]
 
 
 class bte_params(C.Structure):
@@ -109,8 +109,8 @@ def _check(rc: int):
         raise BteError(rc, load_library().bte_last_error().decode())
 
 
-def make_grid(n_harm: int, n_phiy: int, n_batch: int, dt: float) -> bte_grid:
-    return bte_grid(int(n_harm), int(n_phiy), int(n_batch), 0, float(dt))
+def make_grid(n_harm: int, n_phiy: int, n_batch: int, dt: float, precision: int = 0) -> bte_grid:
+    return bte_grid(int(n_harm), int(n_phiy), int(n_batch), int(precision), float(dt))
 
 
 def make_params(ps: Sequence) -> C.Array:
@@ -150,9 +150,10 @@ class Solver:
 
     `grid` has n_harm, n_phiy, n_batch, dt; `params` is a sequence of objects with the fields of
     bte_params (e.g. workloads.Params).  The workspace tensor lives on `device` (default cuda:0).
+    precision: 0 = fp64 (default), 1 = fp32 storage / fp64 arithmetic, 2 = fp32 throughout (bte_grid.precision).
     """
 
-    def __init__(self, grid, params: Sequence, device: str = "cuda:0", stream=None):
+    def __init__(self, grid, params: Sequence, device: str = "cuda:0", stream=None, precision: int = 0):
         import torch  # device memory and streams only
         lib = load_library()
         if not torch.cuda.is_available():
@@ -160,7 +161,7 @@ class Solver:
         if len(params) != grid.n_batch:
             raise ValueError("len(params) must equal grid.n_batch")
         self._lib = lib
-        self.grid = make_grid(grid.n_harm, grid.n_phiy, grid.n_batch, grid.dt)
+        self.grid = make_grid(grid.n_harm, grid.n_phiy, grid.n_batch, grid.dt, precision)
         self.n_harm, self.n_phiy, self.n_batch, self.dt = grid.n_harm, grid.n_phiy, grid.n_batch, grid.dt
         self.shape = (grid.n_harm + 1, grid.n_phiy)
         nbytes = int(lib.bte_workspace_bytes(C.byref(self.grid)))

@@ -4,6 +4,7 @@
 #include "bte_sweep.cuh"
 #include "bte_resident.cuh"
 #include "bte_pendulum.cuh"
+#include "bte_lowprec.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -47,7 +48,7 @@ struct Offsets {
 
 bool grid_ok(const bte_grid* g) {
     return g && g->n_harm >= 1 && g->n_phiy >= 3 && g->n_batch >= 1 && g->n_batch <= 65535 &&
-           g->n_harm < 65535 && g->dt > 0.0 && std::isfinite(g->dt);
+           g->n_harm < 65535 && g->dt > 0.0 && std::isfinite(g->dt) && g->precision >= 0 && g->precision <= 2;
 }
 
 // resident (on-chip) variant: at most RES_MAX_CTAS slabs; usable shared memory per CTA (227 KB minus the
@@ -56,7 +57,7 @@ constexpr int RES_MAX_CTAS = 148;
 constexpr size_t RES_SMEM_CAP = 227 * 1024 - 1024;
 
 bool resident_possible(const bte_grid* g) {
-    if (g->n_batch != 1) return false;
+    if (g->n_batch != 1 || g->precision != 0) return false;   // fp64 only
     const int wc = (g->n_phiy + RES_MAX_CTAS - 1) / RES_MAX_CTAS;
     return resident_smem_bytes(g->n_harm, wc) <= RES_SMEM_CAP;
 }
@@ -66,8 +67,9 @@ Offsets offsets_for(const bte_grid* g) {
     o.pitch = (g->n_phiy + 7) / 8 * 8;
     const size_t rows = (size_t)g->n_harm + 1 + 2 * GHOST, nb = (size_t)g->n_batch, pitch = (size_t)o.pitch;
     size_t off = 0;
-    o.state = off;   off = align_up(off + 2 * 2 * nb * rows * pitch * sizeof(double2));
-    o.state_bytes = 2 * 2 * nb * rows * pitch * sizeof(double2);
+    const size_t elem = g->precision == 0 ? sizeof(double2) : sizeof(float2);   // fp32 storage: half the bytes
+    o.state = off;   off = align_up(off + 2 * 2 * nb * rows * pitch * elem);
+    o.state_bytes = 2 * 2 * nb * rows * pitch * elem;
     o.cn = off;      off = align_up(off + nb * rows * sizeof(double));
     o.gm = off;      off = align_up(off + nb * pitch * sizeof(double));
     o.phi = off;     off = align_up(off + nb * pitch * sizeof(double));
@@ -215,6 +217,8 @@ int sweep_wide(const bte_ctx* c, int S) {
 }
 
 int plan_sweep(bte_ctx* c) {
+    for (int S = 0; S <= SWEEP_MAX_STEPS; ++S) c->sw_grid[S] = 0;
+    if (c->grid.precision != 0) return BTE_OK;     // fp32 variants run the split kernels only
     int dev = 0, sms = 0;
     CUDA_TRY(cudaGetDevice(&dev));
     CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -360,6 +364,7 @@ int launch_resident(bte_ctx* c, int64_t n_steps) {
 }
 
 int effective_variant(const bte_ctx* c) {
+    if (c->grid.precision != 0) return VAR_SPLIT;
     if (c->variant == VAR_AUTO) return c->sw_grid[1] > 0 ? VAR_SWEEP : VAR_FUSED;
     if ((c->variant == VAR_SWEEP || c->variant == VAR_RESIDENT) && c->sw_grid[1] == 0) return VAR_FUSED;
     if (c->variant == VAR_RESIDENT) return VAR_SWEEP;   // what runs when the resident kernel is not used
@@ -402,9 +407,19 @@ int launch_steps(bte_ctx* c, int S) {
         fused_step_kernel<FT, FD><<<c->fgrid, FT, FCfg::smem_bytes, c->stream>>>(c->L, c->rows_per_chunk);
     } else {
         const dim3 g = split_grid(c);
-        half_update_kernel<<<g, 128, 0, c->stream>>>(c->L, 0);
-        half_update_kernel<<<g, 128, 0, c->stream>>>(c->L, 1);
-        reduce_finalize_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 1);
+        if (c->grid.precision == 0) {
+            half_update_kernel<<<g, 128, 0, c->stream>>>(c->L, 0);
+            half_update_kernel<<<g, 128, 0, c->stream>>>(c->L, 1);
+            reduce_finalize_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 1);
+        } else if (c->grid.precision == 1) {
+            half_update32_kernel<1><<<g, 128, 0, c->stream>>>(c->L, 0);
+            half_update32_kernel<1><<<g, 128, 0, c->stream>>>(c->L, 1);
+            reduce_finalize32_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 1);
+        } else {
+            half_update32_kernel<2><<<g, 128, 0, c->stream>>>(c->L, 0);
+            half_update32_kernel<2><<<g, 128, 0, c->stream>>>(c->L, 1);
+            reduce_finalize32_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 1);
+        }
     }
     CUDA_TRY(cudaGetLastError());
     c->launches += launches_per_step(c);
@@ -443,9 +458,12 @@ int build_graph(bte_ctx* c, int64_t len, int S) {
             void* a0[] = {&c->L, &mode0};
             void* a1[] = {&c->L, &mode1};
             void* a2[] = {&c->L, &adv};
-            CUDA_TRY(add((void*)half_update_kernel, g, dim3(128), 0, a0));
-            CUDA_TRY(add((void*)half_update_kernel, g, dim3(128), 0, a1));
-            CUDA_TRY(add((void*)reduce_finalize_kernel, dim3(c->grid.n_batch), dim3(256), 0, a2));
+            void* hu = c->grid.precision == 0 ? (void*)half_update_kernel
+                       : c->grid.precision == 1 ? (void*)half_update32_kernel<1> : (void*)half_update32_kernel<2>;
+            void* rf = c->grid.precision == 0 ? (void*)reduce_finalize_kernel : (void*)reduce_finalize32_kernel;
+            CUDA_TRY(add(hu, g, dim3(128), 0, a0));
+            CUDA_TRY(add(hu, g, dim3(128), 0, a1));
+            CUDA_TRY(add(rf, dim3(c->grid.n_batch), dim3(256), 0, a2));
         }
     }
     CUDA_TRY(cudaGraphInstantiate(&c->graph_exec, c->graph, 0));
@@ -493,8 +511,8 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
                void* cuda_stream, bte_ctx** out) {
     if (out) *out = nullptr;
     if (!out || !grid || !params || !workspace) return fail(BTE_EINVAL, "bte_create: NULL argument");
-    if (!grid_ok(grid) || grid->reserved != 0)
-        return fail(BTE_EINVAL, "bte_create: need n_harm >= 1, n_phiy >= 3, 1 <= n_batch <= 65535, dt > 0");
+    if (!grid_ok(grid))
+        return fail(BTE_EINVAL, "bte_create: need n_harm >= 1, n_phiy >= 3, 1 <= n_batch <= 65535, dt > 0, precision 0..2");
     const Offsets off = offsets_for(grid);
     if (((long long)grid->n_harm + 1 + 2 * GHOST) * off.pitch >= (1LL << 31) - 8LL * off.pitch)
         return fail(BTE_EINVAL, "bte_create: (n_harm+1) * n_phiy must stay below 2^31 points per system");
@@ -601,9 +619,16 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
 int bte_init_equilibrium(bte_ctx* c) {
     if (!c) return fail(BTE_EINVAL, "bte_init_equilibrium: NULL ctx");
     const dim3 g((unsigned)((c->off.pitch + 127) / 128), (unsigned)(c->grid.n_harm + 1), (unsigned)c->grid.n_batch);
-    init_state_kernel<<<g, 128, 0, c->stream>>>(c->L);
-    half_update_kernel<<<split_grid(c), 128, 0, c->stream>>>(c->L, 2);   // start-up z^{1/2}, L202
-    reduce_finalize_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 0);
+    if (c->grid.precision == 0) {
+        init_state_kernel<<<g, 128, 0, c->stream>>>(c->L);
+        half_update_kernel<<<split_grid(c), 128, 0, c->stream>>>(c->L, 2);   // start-up z^{1/2}, L202
+        reduce_finalize_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 0);
+    } else {
+        init_state32_kernel<<<g, 128, 0, c->stream>>>(c->L, c->grid.precision);
+        if (c->grid.precision == 1) half_update32_kernel<1><<<split_grid(c), 128, 0, c->stream>>>(c->L, 2);
+        else half_update32_kernel<2><<<split_grid(c), 128, 0, c->stream>>>(c->L, 2);
+        reduce_finalize32_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 0);
+    }
     CUDA_TRY(cudaGetLastError());
     c->launches += 3;
     c->steps_issued = 0;
@@ -680,6 +705,12 @@ int bte_destroy(bte_ctx* c) {
     return BTE_OK;
 }
 
+// element offset (in lattice points) of row 0 of one (buffer, grid, system) array inside the state region
+size_t state_offset(const bte_ctx* c, int buf, int grid_id, int system) {
+    const size_t gp = (size_t)(c->grid.n_harm + 1 + 2 * GHOST) * c->off.pitch;
+    return (((size_t)buf * 2 + grid_id) * c->grid.n_batch + system) * gp + (size_t)GHOST * c->off.pitch;
+}
+
 int bte_get_state(bte_ctx* c, int32_t system, int32_t grid_id, double* a, double* b) {
     if (!c || !a || !b) return fail(BTE_EINVAL, "bte_get_state: NULL argument");
     if (system < 0 || system >= c->grid.n_batch || grid_id < 0 || grid_id > 1)
@@ -687,17 +718,25 @@ int bte_get_state(bte_ctx* c, int32_t system, int32_t grid_id, double* a, double
     const int rows = c->grid.n_harm + 1, M1 = c->grid.n_phiy, pitch = c->off.pitch;
     int buf = 0;
     { const int rc = live_buffer(c, system, &buf); if (rc != BTE_OK) return rc; }
-    const size_t gp = (size_t)(rows + 2 * GHOST) * pitch, row0 = (size_t)GHOST * pitch;
-    const double2* z = c->L.state + (((size_t)buf * 2 + grid_id) * c->grid.n_batch + system) * gp + row0;
-    // rows 0..N of the other buffer of this (grid, system) are dead between steps: use them as staging
-    double* stage = (double*)(c->L.state + (((size_t)(buf ^ 1) * 2 + grid_id) * c->grid.n_batch + system) * gp + row0);
     const size_t cnt = (size_t)rows * M1;
     const dim3 g((unsigned)((M1 + 255) / 256), (unsigned)rows);
-    deinterleave_kernel<<<g, 256, 0, c->stream>>>(z, stage, stage + cnt, rows, M1, pitch);
+    double *stage_a, *stage_b;
+    // rows 0..N of the other buffer of this system are dead between steps: they serve as staging
+    if (c->grid.precision == 0) {
+        const double2* z = c->L.state + state_offset(c, buf, grid_id, system);
+        stage_a = (double*)(c->L.state + state_offset(c, buf ^ 1, grid_id, system));
+        stage_b = stage_a + cnt;
+        deinterleave_kernel<<<g, 256, 0, c->stream>>>(z, stage_a, stage_b, rows, M1, pitch);
+    } else {   // fp32 arrays hold 8 B per point: a is staged in the dead whole-grid array, b in the fractional one
+        const float2* z = (const float2*)c->L.state + state_offset(c, buf, grid_id, system);
+        stage_a = (double*)((float2*)c->L.state + state_offset(c, buf ^ 1, 0, system));
+        stage_b = (double*)((float2*)c->L.state + state_offset(c, buf ^ 1, 1, system));
+        deinterleave32_kernel<<<g, 256, 0, c->stream>>>(z, stage_a, stage_b, rows, M1, pitch);
+    }
     CUDA_TRY(cudaGetLastError());
     c->launches += 1;
-    CUDA_TRY(cudaMemcpyAsync(a, stage, cnt * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
-    CUDA_TRY(cudaMemcpyAsync(b, stage + cnt, cnt * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaMemcpyAsync(a, stage_a, cnt * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaMemcpyAsync(b, stage_b, cnt * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(cudaStreamSynchronize(c->stream));
     return BTE_OK;
 }
@@ -709,18 +748,27 @@ int bte_set_state(bte_ctx* c, int32_t system, int32_t grid_id, const double* a, 
     const int rows = c->grid.n_harm + 1, M1 = c->grid.n_phiy, pitch = c->off.pitch;
     int buf = 0;
     { const int rc = live_buffer(c, system, &buf); if (rc != BTE_OK) return rc; }
-    const size_t gp = (size_t)(rows + 2 * GHOST) * pitch, row0 = (size_t)GHOST * pitch;
-    double2* z = c->L.state + (((size_t)buf * 2 + grid_id) * c->grid.n_batch + system) * gp + row0;
-    double* stage = (double*)(c->L.state + (((size_t)(buf ^ 1) * 2 + grid_id) * c->grid.n_batch + system) * gp + row0);
     const size_t cnt = (size_t)rows * M1;
-    CUDA_TRY(cudaMemcpyAsync(stage, a, cnt * sizeof(double), cudaMemcpyHostToDevice, c->stream));
-    CUDA_TRY(cudaMemcpyAsync(stage + cnt, b, cnt * sizeof(double), cudaMemcpyHostToDevice, c->stream));
     const dim3 g((unsigned)((pitch + 255) / 256), (unsigned)rows);
-    interleave_kernel<<<g, 256, 0, c->stream>>>(z, stage, stage + cnt, rows, M1, pitch);
+    if (c->grid.precision == 0) {
+        double2* z = c->L.state + state_offset(c, buf, grid_id, system);
+        double* stage = (double*)(c->L.state + state_offset(c, buf ^ 1, grid_id, system));
+        CUDA_TRY(cudaMemcpyAsync(stage, a, cnt * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+        CUDA_TRY(cudaMemcpyAsync(stage + cnt, b, cnt * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+        interleave_kernel<<<g, 256, 0, c->stream>>>(z, stage, stage + cnt, rows, M1, pitch);
+    } else {
+        float2* z = (float2*)c->L.state + state_offset(c, buf, grid_id, system);
+        double* stage_a = (double*)((float2*)c->L.state + state_offset(c, buf ^ 1, 0, system));
+        double* stage_b = (double*)((float2*)c->L.state + state_offset(c, buf ^ 1, 1, system));
+        CUDA_TRY(cudaMemcpyAsync(stage_a, a, cnt * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+        CUDA_TRY(cudaMemcpyAsync(stage_b, b, cnt * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+        interleave32_kernel<<<g, 256, 0, c->stream>>>(z, stage_a, stage_b, rows, M1, pitch);
+    }
     c->launches += 1;
     if (grid_id == 0) {   // keep norm / v_dr of the observables consistent with the new whole grid
-        // reduce_finalize reads the live buffer of every system; harmless for the others
-        reduce_finalize_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 0);
+        // the reduction reads the live buffer of every system; harmless for the others
+        if (c->grid.precision == 0) reduce_finalize_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 0);
+        else reduce_finalize32_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 0);
         c->launches += 1;
     }
     CUDA_TRY(cudaGetLastError());
@@ -733,6 +781,7 @@ int bte_reconstruct_pdf(bte_ctx* c, int32_t system, int32_t grid_id, int32_t n_p
     if (system < 0 || system >= c->grid.n_batch || grid_id < 0 || grid_id > 1)
         return fail(BTE_EINVAL, "bte_reconstruct_pdf: bad system or grid index");
     if (n_phix < 1 || n_phix > 2048) return fail(BTE_EINVAL, "bte_reconstruct_pdf: n_phix must be in [1, 2048]");
+    if (c->grid.precision != 0) return fail(BTE_EINVAL, "bte_reconstruct_pdf: fp64 contexts only");
     const int rows = c->grid.n_harm + 1, M1 = c->grid.n_phiy, pitch = c->off.pitch;
     int buf = 0;
     { const int rc = live_buffer(c, system, &buf); if (rc != BTE_OK) return rc; }
