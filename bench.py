@@ -196,7 +196,7 @@ def run_ours(args):
         return _max_over_ranks(x, dev)
 
     # ---- device-resident measurement: inputs (state) already in HBM ---------------------------------
-    s = Solver(w.grid, w.params, device=dev)
+    s = Solver(w.grid, w.params, device=dev, precision=args.precision)
     if args.variant:
         s.set_option("variant", args.variant)
     if args.tile_rows:
@@ -277,7 +277,7 @@ def run_ours(args):
     host_in = torch.empty((nb, 2, 2) + shape, dtype=torch.float64).pin_memory()
     host_out = torch.empty((nb, 2, 2) + shape, dtype=torch.float64).pin_memory()
     hin, hout = host_in.numpy(), host_out.numpy()
-    s1 = Solver(w.grid, w.params, device=dev)        # untimed: produce the t = 0 state on the host
+    s1 = Solver(w.grid, w.params, device=dev, precision=args.precision)   # untimed: the t = 0 state on the host
     s1.init_equilibrium()
     for i in range(nb):
         for g in (0, 1):
@@ -286,7 +286,7 @@ def run_ours(args):
     del s1
     barrier()
     t0 = time.perf_counter()
-    s2 = Solver(w.grid, w.params, device=dev)
+    s2 = Solver(w.grid, w.params, device=dev, precision=args.precision)
     configure(s2)
     for i in range(nb):
         for g in (0, 1):
@@ -324,7 +324,8 @@ def run_ours(args):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None,
+        "dtype": ("f64", "f32 storage / f64 arithmetic", "f32")[args.precision], "data": "synthetic",
         "config": {"workload": w.name, **w.describe(), "state_bytes": 32 * pts_all,
                    "l2_policy": (f"inputs larger than L2 ({32 * pts_all / 1e6:.0f} MB state vs 126 MB L2)"
                                  if 32 * pts_all > 2.6e8 else
@@ -381,6 +382,9 @@ def main():
     ap.add_argument("--tile-rows", type=int, default=0)
     ap.add_argument("--sweep-steps", type=int, default=0, help="steps fused per launch (0 auto)")
     ap.add_argument("--ctas", type=int, default=0, help="persistent CTAs of the sweep kernel (0 auto)")
+    ap.add_argument("--precision", type=int, default=0, choices=[0, 1, 2],
+                    help="0 fp64 (the metric); 1 fp32 storage / fp64 arithmetic, 2 fp32 throughout (NEXT-4 variants, "
+                         "two launches per step; reported with dtype f32 -- not the BASELINE metric)")
     ap.add_argument("--sweep-threads", type=int, default=0, help="threads per CTA of the sweep kernel (0 auto)")
     ap.add_argument("--res-ctas", type=int, default=0, help="slabs of the resident kernel (0 auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")

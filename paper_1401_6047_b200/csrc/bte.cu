@@ -394,6 +394,13 @@ dim3 split_grid(const bte_ctx* c) {
                 (unsigned)c->grid.n_batch);
 }
 
+// column chunks x systems of reduce_finalize_kernel (each chunk at least one block's worth of columns)
+dim3 reduce_grid(const bte_ctx* c) {
+    int nb = (c->grid.n_phiy + 255) / 256;
+    if (nb > RED_BLOCKS) nb = RED_BLOCKS;
+    return dim3((unsigned)nb, (unsigned)c->grid.n_batch);
+}
+
 int launches_per_step(const bte_ctx* c) { return effective_variant(c) == VAR_SPLIT ? 3 : 1; }
 
 // Issue one launch group with plain launches: S steps (sweep kernel) or one step (other variants).
@@ -410,15 +417,15 @@ int launch_steps(bte_ctx* c, int S) {
         if (c->grid.precision == 0) {
             half_update_kernel<<<g, 128, 0, c->stream>>>(c->L, 0);
             half_update_kernel<<<g, 128, 0, c->stream>>>(c->L, 1);
-            reduce_finalize_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 1);
+            reduce_finalize_kernel<double2><<<reduce_grid(c), 256, 0, c->stream>>>(c->L, 1);
         } else if (c->grid.precision == 1) {
             half_update32_kernel<1><<<g, 128, 0, c->stream>>>(c->L, 0);
             half_update32_kernel<1><<<g, 128, 0, c->stream>>>(c->L, 1);
-            reduce_finalize32_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 1);
+            reduce_finalize_kernel<float2><<<reduce_grid(c), 256, 0, c->stream>>>(c->L, 1);
         } else {
             half_update32_kernel<2><<<g, 128, 0, c->stream>>>(c->L, 0);
             half_update32_kernel<2><<<g, 128, 0, c->stream>>>(c->L, 1);
-            reduce_finalize32_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 1);
+            reduce_finalize_kernel<float2><<<reduce_grid(c), 256, 0, c->stream>>>(c->L, 1);
         }
     }
     CUDA_TRY(cudaGetLastError());
@@ -460,10 +467,10 @@ int build_graph(bte_ctx* c, int64_t len, int S) {
             void* a2[] = {&c->L, &adv};
             void* hu = c->grid.precision == 0 ? (void*)half_update_kernel
                        : c->grid.precision == 1 ? (void*)half_update32_kernel<1> : (void*)half_update32_kernel<2>;
-            void* rf = c->grid.precision == 0 ? (void*)reduce_finalize_kernel : (void*)reduce_finalize32_kernel;
+            void* rf = c->grid.precision == 0 ? (void*)reduce_finalize_kernel<double2> : (void*)reduce_finalize_kernel<float2>;
             CUDA_TRY(add(hu, g, dim3(128), 0, a0));
             CUDA_TRY(add(hu, g, dim3(128), 0, a1));
-            CUDA_TRY(add(rf, dim3(c->grid.n_batch), dim3(256), 0, a2));
+            CUDA_TRY(add(rf, reduce_grid(c), dim3(256), 0, a2));
         }
     }
     CUDA_TRY(cudaGraphInstantiate(&c->graph_exec, c->graph, 0));
@@ -622,12 +629,12 @@ int bte_init_equilibrium(bte_ctx* c) {
     if (c->grid.precision == 0) {
         init_state_kernel<<<g, 128, 0, c->stream>>>(c->L);
         half_update_kernel<<<split_grid(c), 128, 0, c->stream>>>(c->L, 2);   // start-up z^{1/2}, L202
-        reduce_finalize_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 0);
+        reduce_finalize_kernel<double2><<<reduce_grid(c), 256, 0, c->stream>>>(c->L, 0);
     } else {
         init_state32_kernel<<<g, 128, 0, c->stream>>>(c->L, c->grid.precision);
         if (c->grid.precision == 1) half_update32_kernel<1><<<split_grid(c), 128, 0, c->stream>>>(c->L, 2);
         else half_update32_kernel<2><<<split_grid(c), 128, 0, c->stream>>>(c->L, 2);
-        reduce_finalize32_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 0);
+        reduce_finalize_kernel<float2><<<reduce_grid(c), 256, 0, c->stream>>>(c->L, 0);
     }
     CUDA_TRY(cudaGetLastError());
     c->launches += 3;
@@ -767,8 +774,8 @@ int bte_set_state(bte_ctx* c, int32_t system, int32_t grid_id, const double* a, 
     c->launches += 1;
     if (grid_id == 0) {   // keep norm / v_dr of the observables consistent with the new whole grid
         // the reduction reads the live buffer of every system; harmless for the others
-        if (c->grid.precision == 0) reduce_finalize_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 0);
-        else reduce_finalize32_kernel<<<c->grid.n_batch, 256, 0, c->stream>>>(c->L, 0);
+        if (c->grid.precision == 0) reduce_finalize_kernel<double2><<<reduce_grid(c), 256, 0, c->stream>>>(c->L, 0);
+        else reduce_finalize_kernel<float2><<<reduce_grid(c), 256, 0, c->stream>>>(c->L, 0);
         c->launches += 1;
     }
     CUDA_TRY(cudaGetLastError());

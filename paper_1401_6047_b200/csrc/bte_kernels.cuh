@@ -151,35 +151,51 @@ __global__ void __launch_bounds__(128) half_update_kernel(Layout L, int mode) {
     O[n * p + m] = w;
 }
 
-// One block per system: sums row 0 (a) and row 1 (b) of the whole grid in buffer (buf ^ advance),
-// then folds.  Used by the split variant (advance = 1) and after init / set_state (advance = 0).
+// Sums row 0 (a) and row 1 (b) of the whole grid in buffer (buf ^ advance) and folds.  Used by the split variants
+// (advance = 1) and after init / set_state (advance = 0).  grid = (RED_BLOCKS-or-fewer column chunks, n_batch);
+// the last block of a system to finish folds the per-warp partial sums in fixed order (deterministic).
+// E2 = double2 (fp64 state) or float2 (fp32 state, bte_lowprec.cuh); sums accumulate in fp64 either way.
+constexpr int RED_BLOCKS = 64;
+
+template <class E2>
+__device__ __forceinline__ E2* state_ptr_t(const Layout& L, int buf, int grid, int sys) {
+    return (E2*)L.state + (((size_t)buf * 2 + grid) * L.n_batch + sys) * grid_points(L) + (size_t)GHOST * L.pitch;
+}
+
+template <class E2>
 __global__ void __launch_bounds__(256) reduce_finalize_kernel(Layout L, int advance) {
-    const int sys = blockIdx.x;
+    __shared__ unsigned int s_last;
+    const int sys = blockIdx.y;
     const SysConst c = L.sc[sys];
     const long long k = L.ss[sys].k;
     if (advance && c.n_steps_total > 0 && k >= c.n_steps_total) return;
     const int buf = L.ss[sys].buf ^ (advance ? 1 : 0);
-    const double2* H = state_ptr(L, buf, 0, sys);
+    const E2* H = state_ptr_t<E2>(L, buf, 0, sys);
+    const int chunk = (L.M1 + gridDim.x - 1) / gridDim.x;
+    const int m0 = blockIdx.x * chunk, m1 = min(L.M1, m0 + chunk);
     double sa = 0.0, sb = 0.0;
-    for (int m = threadIdx.x; m < L.M1; m += blockDim.x) {
-        sa += H[m].x;
-        sb += H[(size_t)L.pitch + m].y;   // N >= 1 is enforced by bte_create
+    for (int m = m0 + threadIdx.x; m < m1; m += blockDim.x) {
+        sa += (double)H[m].x;
+        sb += (double)H[(size_t)L.pitch + m].y;   // N >= 1 is enforced by bte_create
     }
     sa = warp_sum(sa);
     sb = warp_sum(sb);
     double* part = L.partial + (size_t)sys * L.pitch * 2;
-    const int warp = threadIdx.x >> 5;
+    const int warp = threadIdx.x >> 5, slot = blockIdx.x * 8 + warp;     // 8 warps per block
     if ((threadIdx.x & 31) == 0) {
-        part[2 * warp] = sa;
-        part[2 * warp + 1] = sb;
+        part[2 * slot] = sa;
+        part[2 * slot + 1] = sb;
     }
-    if (threadIdx.x == 0) {
-        L.ss[sys].edge[0] = fabs(H[(size_t)L.pitch].y);
-        L.ss[sys].edge[1] = fabs(H[(size_t)L.pitch + L.M1 - 1].y);
-    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) L.ss[sys].edge[0] = fabs((double)H[(size_t)L.pitch].y);
+    if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) L.ss[sys].edge[1] = fabs((double)H[(size_t)L.pitch + L.M1 - 1].y);
     __threadfence();
     __syncthreads();
-    if (warp == 0) fold_and_advance(L, sys, blockDim.x >> 5, k, advance ? 1 : 0);
+    if (threadIdx.x == 0) s_last = (atomicAdd(&L.ss[sys].done, 1u) + 1u == gridDim.x) ? 1u : 0u;
+    __syncthreads();
+    if (s_last && warp == 0) {
+        __threadfence();
+        fold_and_advance(L, sys, (int)gridDim.x * 8, k, advance ? 1 : 0);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -5,7 +5,7 @@
 //           in float (explicit round-to-nearest intrinsics, no FMA contraction, IEEE division): bit-reproducible
 //           against a CPU float implementation.
 // Kernels: one thread per lattice point, two launches per step plus the reduction (the "split" form of the step;
-// the streaming / resident kernels are fp64-only).  Reductions accumulate in fp64.
+// the streaming / resident kernels are fp64-only).  Reductions (reduce_finalize_kernel<float2>) accumulate in fp64.
 #pragma once
 #include "bte_kernels.cuh"
 
@@ -87,8 +87,8 @@ __global__ void __launch_bounds__(128) half_update32_kernel(Layout L, int mode) 
         const float Ea = (float)Es[0], Eb = (float)Es[1], Bf = (float)c.B, ph = (float)ph_d, nf = (float)n;
         const float beta_a = __fadd_rn(Ea, __fmul_rn(Bf, ph));             // eq. (28)-(29)
         const float beta_b = __fadd_rn(Eb, __fmul_rn(Bf, ph));
-        const float mu_a = __fdiv_rn(__fmul_rn(__fmul_rn(nf, beta_a), d), 2.0f);
-        const float mu_b = __fdiv_rn(__fmul_rn(__fmul_rn(nf, beta_b), d), 2.0f);
+        const float mu_a = __fmul_rn(__fmul_rn(__fmul_rn(nf, beta_a), d), 0.5f);   // x / 2 == x * 0.5 exactly
+        const float mu_b = __fmul_rn(__fmul_rn(__fmul_rn(nf, beta_b), d), 0.5f);
         const float chi = (n == 1) ? 2.0f : 1.0f;                          // eq. (11)
         const float Bt = __fmul_rn(kap, __fadd_rn(__fsub_rn(__fsub_rn(up.y, um.y), lp.y), lm.y));            // eq. (31)
         const float At = __fmul_rn(kap, __fadd_rn(__fsub_rn(__fmul_rn(chi, __fsub_rn(lp.x, lm.x)), up.x), um.x));  // (30)
@@ -101,36 +101,6 @@ __global__ void __launch_bounds__(128) half_update32_kernel(Layout L, int mode) 
     }
     if (n == 0) out.y = 0.f;                                               // b_0 == 0, eq. (23) / C3
     O[n * p + m] = out;
-}
-
-// norm / v_dr / running sums from the fp32 state, accumulated in fp64 (one block per system).
-__global__ void __launch_bounds__(256) reduce_finalize32_kernel(Layout L, int advance) {
-    const int sys = blockIdx.x;
-    const SysConst c = L.sc[sys];
-    const long long k = L.ss[sys].k;
-    if (advance && c.n_steps_total > 0 && k >= c.n_steps_total) return;
-    const int buf = L.ss[sys].buf ^ (advance ? 1 : 0);
-    const float2* H = state32_ptr(L, buf, 0, sys);
-    double sa = 0.0, sb = 0.0;
-    for (int m = threadIdx.x; m < L.M1; m += blockDim.x) {
-        sa += (double)H[m].x;
-        sb += (double)H[(size_t)L.pitch + m].y;
-    }
-    sa = warp_sum(sa);
-    sb = warp_sum(sb);
-    double* part = L.partial + (size_t)sys * L.pitch * 2;
-    const int warp = threadIdx.x >> 5;
-    if ((threadIdx.x & 31) == 0) {
-        part[2 * warp] = sa;
-        part[2 * warp + 1] = sb;
-    }
-    if (threadIdx.x == 0) {
-        L.ss[sys].edge[0] = fabs((double)H[(size_t)L.pitch].y);
-        L.ss[sys].edge[1] = fabs((double)H[(size_t)L.pitch + L.M1 - 1].y);
-    }
-    __threadfence();
-    __syncthreads();
-    if (warp == 0) fold_and_advance(L, sys, blockDim.x >> 5, k, advance ? 1 : 0);
 }
 
 // host (fp64 arrays) <-> fp32 workspace state
