@@ -24,8 +24,14 @@
  *   - Arrays a, b exchanged with the host are row-major (n_harm+1) x n_phiy doubles, m fastest
  *     (the layout of Fig. 7).  Inside the workspace the state is stored as interleaved (a,b)
  *     pairs.
- *   - The library is fp64 throughout.  Work is issued asynchronously on the CUDA stream given at create
+ *   - fp64 throughout unless bte_grid.precision asks for one of the fp32 variants of the step (the paper's own
+ *     precision; reference-grade kernels).  Work is issued asynchronously on the CUDA stream given at create
  *     time (a cudaStream_t passed as void*; NULL = legacy default stream).
+ *   - How a step is executed is chosen automatically (bte_set_option "variant"): lattices that fit the GPU's
+ *     shared memory run the whole time loop of a bte_step call in one launch (resident kernel); larger ones and
+ *     batches stream through HBM once per 2-3 time steps (sweep kernel).  Results do not depend on the choice
+ *     beyond rounding of the sums (the state is bit-identical across variants).
+ *   - Beyond the time step: bte_reconstruct_pdf (eq. 8) and bte_pendulum_averages (eq. 44-46), see below.
  *   - Not thread-safe per ctx; distinct ctxs may be used from distinct threads.
  */
 #ifndef BTE_B200_H

@@ -1,14 +1,17 @@
-// bte_kernels.cuh -- sm_100a kernels of libbte_b200.
+// bte_kernels.cuh -- the simple sm_100a kernels of libbte_b200 (the production step kernels live in
+// bte_sweep.cuh and bte_resident.cuh and include this file).
 //
-//   init_state_kernel      a_h = a^(0) = c_n g_m, b_h = 0                       (eq. 15)
-//   half_update_kernel     one application of T (eq. 38) to one grid: the "split" variant of the step
-//                          (two launches per step, 96 B/point) and the start-up z^{1/2} (L202)
-//   reduce_finalize_kernel norm / v_dr / running sums for the split variant and after init
-//   fused_step_kernel      whole + fractional update in ONE sweep (eq. 40-41), 64 B/point: each CTA
-//                          marches a strip of phi_y columns over the harmonics n, rows staged through a
-//                          shared-memory ring by cp.async (zero-fill = boundary conditions 22-23),
-//                          reductions and the step bookkeeping fused in (last-block-done fold)
-//   (de)interleave kernels host <-> workspace state exchange
+//   init_state_kernel        a_h = a^(0) = c_n g_m, b_h = 0                       (eq. 15)
+//   half_update_kernel       one application of T (eq. 38) to one grid, one thread per lattice point: the
+//                            "split" variant of the step (two launches per step, 96 B/point; cross-check of the
+//                            production kernels) and the start-up z^{1/2} (L202)
+//   reduce_finalize_kernel   norm / v_dr / running sums for the split variants and after init / set_state
+//                            (multi-block, deterministic last-block fold; templated on the state type)
+//   fused_step_kernel        whole + fractional update in ONE sweep over a 2-D tile grid (variant 2, cross-check):
+//                            each CTA marches a strip of phi_y columns over a chunk of harmonics, rows staged
+//                            through a shared-memory ring by cp.async (zero-fill = boundary conditions 22-23)
+//   (de)interleave kernels   host <-> workspace state exchange
+//   pdf_kernel               f(phi_x, phi_y) of eq. (8) from the coefficients
 #pragma once
 #include "bte_device.cuh"
 
