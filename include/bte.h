@@ -152,8 +152,9 @@ int bte_pendulum_averages(const bte_pendulum_params* params, int32_t n, int32_t 
  *                  3 = persistent sweep kernel, S steps per launch (64/S B/point/step; the default path
  *                      for lattices larger than the GPU's shared memory),
  *                  4 = resident kernel: the whole time loop of one bte_step call in ONE launch, state held
- *                      in shared memory (n_batch = 1 and both grids must fit the shared memory of the GPU;
- *                      otherwise variant 3 runs).  Automatic choice: 4 when usable and n_steps >= 4, else 3.
+ *                      in shared memory (one system: both grids must fit the shared memory of the GPU; a batch:
+ *                      each system must fit one cluster of 16 CTAs; otherwise variant 3 runs).  Automatic
+ *                      choice: 4 when usable, n_steps >= 4 and (for a batch) systems of at most 8192 points.
  *   "resident_ctas" slabs (CTAs) of variant 4: 1 = one CTA, 2..16 = one thread-block cluster, more = cooperative
  *                  grid; 0 = automatic
  *   "sweep_steps"  S of variant 3: 1..3, 0 = automatic

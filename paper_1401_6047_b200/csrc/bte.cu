@@ -55,10 +55,13 @@ bool grid_ok(const bte_grid* g) {
 // kernel's static shared memory)
 constexpr int RES_MAX_CTAS = 148;
 constexpr size_t RES_SMEM_CAP = 227 * 1024 - 1024;
+constexpr long long RES_BATCH_MAX_POINTS = 8192;   // automatic choice for batches: systems up to this many points
 
 bool resident_possible(const bte_grid* g) {
-    if (g->n_batch != 1 || g->precision != 0) return false;   // fp64 only
-    const int wc = (g->n_phiy + RES_MAX_CTAS - 1) / RES_MAX_CTAS;
+    if (g->precision != 0) return false;                       // fp64 only
+    // one system: up to RES_MAX_CTAS slabs (cooperative grid); a batch: one cluster of up to 16 CTAs per system
+    const int gmax = g->n_batch == 1 ? RES_MAX_CTAS : 16;
+    const int wc = (g->n_phiy + gmax - 1) / gmax;
     return resident_smem_bytes(g->n_harm, wc) <= RES_SMEM_CAP;
 }
 
@@ -79,8 +82,9 @@ Offsets offsets_for(const bte_grid* g) {
     o.gctl = off;    off = align_up(off + 64);
     // resident variant: edge columns of both grids of every slab, per-slab sums
     o.rhalo = off;
-    if (resident_possible(g)) off = align_up(off + (size_t)2 * RES_MAX_CTAS * 2 * (g->n_harm + 1) * sizeof(double2));
-    o.rout = off;    off = align_up(off + (size_t)RES_MAX_CTAS * 8 * sizeof(double));
+    if (resident_possible(g) && g->n_batch == 1)
+        off = align_up(off + (size_t)2 * RES_MAX_CTAS * 2 * (g->n_harm + 1) * sizeof(double2));
+    o.rout = off;    off = align_up(off + std::max<size_t>(RES_MAX_CTAS, (size_t)g->n_batch * 16) * 8 * sizeof(double));
     o.rflag = off;   off = align_up(off + (size_t)RES_MAX_CTAS * sizeof(unsigned int));
     o.total = off;
     return o;
@@ -320,7 +324,7 @@ int plan_resident(bte_ctx* c) {
         const int G = c->res_ctas_opt;
         if (G == 1) resident_try(c, 0, 1);
         else if (G <= 16 && resident_try(c, 1, G)) {}
-        else if (G <= maxg) resident_try(c, 2, G);
+        else if (G <= maxg && c->grid.n_batch == 1) resident_try(c, 2, G);
         return BTE_OK;
     }
     // automatic: the fewest slabs that leave about one point per thread (synchronisation cost grows with the
@@ -331,7 +335,7 @@ int plan_resident(bte_ctx* c) {
     for (int G = 8; G >= 2; G /= 2)             // 16 not schedulable / does not fit: smaller clusters that fit
         if (resident_try(c, 1, G)) return BTE_OK;
     if (resident_try(c, 0, 1)) return BTE_OK;
-    resident_try(c, 2, maxg);
+    if (c->grid.n_batch == 1) resident_try(c, 2, maxg);    // the grid mode synchronises CTAs of ONE system
     return BTE_OK;
 }
 
@@ -344,7 +348,8 @@ int launch_resident(bte_ctx* c, int64_t n_steps) {
     void* fn = resident_fn(c->res_mode);
     void* args[] = {&c->L, &A};
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3(c->res_G); cfg.blockDim = dim3(c->res_T + 32); cfg.dynamicSmemBytes = c->res_smem;
+    cfg.gridDim = dim3((unsigned)c->res_G * (unsigned)c->grid.n_batch);   // one CTA / cluster per system
+    cfg.blockDim = dim3(c->res_T + 32); cfg.dynamicSmemBytes = c->res_smem;
     cfg.stream = c->stream;
     cudaLaunchAttribute at[1];
     cfg.attrs = at; cfg.numAttrs = 0;
@@ -648,10 +653,15 @@ int bte_step(bte_ctx* c, int64_t n_steps) {
     int64_t left = n_steps;
     // lattices that fit on chip: ONE launch runs the whole time loop out of shared memory (automatic choice
     // from 4 steps on -- below that the load/store of the state is not amortised)
-    if (c->res_mode >= 0 && (c->variant == VAR_RESIDENT || (c->variant == VAR_AUTO && n_steps >= 4))) {
-        const int64_t tot = c->params[0].n_steps_total;
+    // (batches: only small systems -- a batch of mid-size systems streams faster through the sweep kernel)
+    const bool res_auto = c->variant == VAR_AUTO && n_steps >= 4 &&
+                          (c->grid.n_batch == 1 || (long long)(c->grid.n_harm + 1) * c->grid.n_phiy <= RES_BATCH_MAX_POINTS);
+    if (c->res_mode >= 0 && (c->variant == VAR_RESIDENT || res_auto)) {
         int64_t n = n_steps;
-        if (tot > 0) n = std::min<int64_t>(n, std::max<int64_t>(0, tot - c->steps_issued));
+        if (c->grid.n_batch == 1) {            // (a batch: the kernel ends every system at its own budget)
+            const int64_t tot = c->params[0].n_steps_total;
+            if (tot > 0) n = std::min<int64_t>(n, std::max<int64_t>(0, tot - c->steps_issued));
+        }
         while (n > 0) {                      // 32-bit half-update counters inside the kernel: <= 2^30 steps a launch
             const int64_t m = std::min<int64_t>(n, (int64_t)1 << 30);
             const int rc = launch_resident(c, m);

@@ -1,6 +1,7 @@
 // bte_resident.cuh -- on-chip time loop for lattices that fit the shared memory of the GPU (sm_100a).
 //
-// One launch = ALL n_steps leap-frog steps (eq. 40-41) of one system.  The phi_y axis is cut into G slabs of
+// One launch = ALL n_steps leap-frog steps (eq. 40-41) of every system of the batch (one CTA or one thread-block
+// cluster per system; clusters are independent, the hardware schedules them as SMs become free).  The phi_y axis is cut into G slabs of
 // Wc columns; CTA g keeps its slab of BOTH grids (whole and fractional, all harmonics n = 0..N) in shared
 // memory for the whole launch, with one halo column on each side and one zero ghost row above and below
 // (the zero perimeter of PAPER.md:L278, i.e. eq. 22-23).  HBM is touched twice: the state is loaded at the
@@ -28,9 +29,9 @@ struct ResidentArgs {
     int G;                 // slabs = CTAs
     int Wc;                // columns per slab (the last slab may hold fewer valid columns)
     int T;                 // compute threads per CTA (blockDim.x = T + 32: one more warp does the bookkeeping)
-    long long n_steps;     // steps of this launch (>= 1)
+    long long n_steps;     // steps of this launch (>= 1); a system's step budget may end it earlier
     double2* halo;         // MODE 2: [grid 2][G][side 2][N+1] edge columns
-    double* cta_out;       // [G][8] per-slab results at the end of the launch
+    double* cta_out;       // [n_batch][G][8] per-slab results at the end of the launch
     unsigned int* flag;    // MODE 2: [G] half-updates completed by each CTA (zeroed by the host before a launch)
 };
 
@@ -115,11 +116,11 @@ __global__ void __launch_bounds__(1024, 1) resident_kernel(const __grid_constant
     const int tid = threadIdx.x, T = A.T, NT = blockDim.x;
     const bool service = tid >= T;        // last warp: tables and the running sums, no lattice points
     const int lane = tid & 31, warp = tid >> 5;
-    const int g = blockIdx.x, G = A.G, Wc = A.Wc;
+    const int G = A.G, Wc = A.Wc;
+    const int sys = blockIdx.x / G, g = blockIdx.x - sys * G;   // batches: one CTA / one cluster per system
     const int N = L.N, rows = N + 1, P = Wc + 2;
     const int c0 = g * Wc;
     const int Wv = min(Wc, L.M1 - c0);    // valid columns of this slab (>= 1 by construction of the plan)
-    const int sys = 0;
 
     double2* Hs = smem;
     double2* Fs = smem + (size_t)(N + 3) * P;
@@ -130,6 +131,10 @@ __global__ void __launch_bounds__(1024, 1) resident_kernel(const __grid_constant
     const SysConst c = L.sc[sys];
     const long long k0 = L.ss[sys].k;
     const int buf = L.ss[sys].buf;
+    // steps of this launch for this system: a step budget may end it early (uniform over the system's CTAs)
+    const long long n_steps = c.n_steps_total > 0 ? max(0LL, min((long long)A.n_steps, c.n_steps_total - k0))
+                                                  : (long long)A.n_steps;
+    if (n_steps == 0) return;
     double2* __restrict__ Hg = state_ptr(L, buf, 0, sys);
     double2* __restrict__ Fg = state_ptr(L, buf, 1, sys);
     auto E_at = [&](long long q) {        // E at half-step q of this launch
@@ -182,7 +187,7 @@ __global__ void __launch_bounds__(1024, 1) resident_kernel(const __grid_constant
     double A_last = 0.0, B_last = 0.0, SV = 0.0, SC = 0.0, SS = 0.0;
     double window = L.ss[sys].window;     // advanced by repeated addition of dt, like the step-by-step kernels
 
-    for (long long q = 0; q < 2 * A.n_steps; ++q) {
+    for (long long q = 0; q < 2 * n_steps; ++q) {
         const bool whole = (q & 1) == 0;
         double2* X = whole ? Hs : Fs;
         const unsigned done = (unsigned)q + 1u;
@@ -273,11 +278,11 @@ __global__ void __launch_bounds__(1024, 1) resident_kernel(const __grid_constant
     if (g == 0 && tid == 0) L.ss[sys].edge[0] = fabs(Hs[2 * P + 1].y);          // |b_{1,0}|   (C12)
     if (g == G - 1 && tid == 0) L.ss[sys].edge[1] = fabs(Hs[2 * P + Wv].y);     // |b_{1,M}|
     if (service && lane == 0) {
-        double* o = A.cta_out + (size_t)g * 8;
+        double* o = A.cta_out + (size_t)blockIdx.x * 8;
         o[0] = A_last; o[1] = B_last; o[2] = SV; o[3] = SC; o[4] = SS; o[5] = window;
     }
     // ---- one launch-wide synchronisation, then CTA 0 adds the slabs in a fixed order --------------------------
-    const unsigned fin = (unsigned)(2 * A.n_steps) + 1u;
+    const unsigned fin = (unsigned)(2 * n_steps) + 1u;
     if (MODE == 0) {
         __syncthreads();
     } else if (MODE == 1) {
@@ -300,7 +305,7 @@ __global__ void __launch_bounds__(1024, 1) resident_kernel(const __grid_constant
         double t[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
         for (int s = lane; s < G; s += 32) {
 #pragma unroll
-            for (int x = 0; x < 5; ++x) t[x] += __ldcg(A.cta_out + (size_t)s * 8 + x);
+            for (int x = 0; x < 5; ++x) t[x] += __ldcg(A.cta_out + ((size_t)sys * G + s) * 8 + x);
         }
 #pragma unroll
         for (int x = 0; x < 5; ++x) t[x] = warp_sum(t[x]);
@@ -311,9 +316,9 @@ __global__ void __launch_bounds__(1024, 1) resident_kernel(const __grid_constant
             st->sum_v += c.v_scale * t[2] * L.dt;               // eq. (17) sums, C9
             st->sum_c += c.v_scale * t[3] * L.dt;
             st->sum_s += c.v_scale * t[4] * L.dt;
-            st->window = __ldcg(A.cta_out + 5);
+            st->window = __ldcg(A.cta_out + (size_t)sys * G * 8 + 5);
             st->edge_leak = ((volatile double*)st->edge)[0] + ((volatile double*)st->edge)[1];
-            st->k = k0 + A.n_steps;
+            st->k = k0 + n_steps;
         }
     }
 }

@@ -140,6 +140,40 @@ def test_resident_slabs(res_ctas):
     s.destroy()
 
 
+@pytest.mark.parametrize("res_ctas", [1, 2, 4, 0])
+def test_resident_batched_with_budgets(res_ctas):
+    """A batch on the resident kernel: one CTA / one cluster per system, every system ends at its own step budget;
+    several bte_step calls; more systems than SMs would also just queue (clusters are independent)."""
+    w = W.random_batch(n_batch=9, N=9, M1=140, dt=0.004, seed=31, periods=0.2)
+    n = w.n_steps + 3
+    s = gpu_solver(w, "resident", res_ctas=res_ctas)
+    n0 = s.launch_count()
+    s.step(n // 3); s.step(n - n // 3)
+    assert s.launch_count() - n0 == 2
+    obs = s.observables()
+    sims = oracle_run(w, n)
+    for i, sim in sims.items():
+        assert obs[i].step == w.params[i].n_steps_total
+        assert_state_close(s, sim, i, what=f"resident batch[{i}] ctas={res_ctas}")
+        assert_obs_close(obs[i], sim.observables(), w.params[i], w.grid.dt, what=f"resident batch[{i}] ctas={res_ctas}")
+    s.destroy()
+
+
+def test_resident_batch_of_many_small_systems_auto():
+    """200 systems of 5 x 33 points (more clusters than SMs), automatic variant choice = resident; a sample is
+    compared with the oracle."""
+    w = W.random_batch(n_batch=200, N=4, M1=33, dt=0.004, seed=5, periods=0.0, n_steps=60)
+    s = gpu_solver(w, "auto")
+    n0 = s.launch_count()
+    s.step(60)
+    assert s.launch_count() - n0 == 1
+    obs = s.observables()
+    for i, sim in oracle_run(w, 60, systems=[0, 57, 131, 199]).items():
+        assert_state_close(s, sim, i, what=f"many small[{i}]")
+        assert_obs_close(obs[i], sim.observables(), w.params[i], w.grid.dt, what=f"many small[{i}]")
+    s.destroy()
+
+
 def test_resident_interleaves_with_sweep_and_budget():
     """The resident kernel and the streaming kernels share the state: alternate them; a step budget freezes
     the system exactly at n_steps_total."""
