@@ -146,6 +146,30 @@ size_t bte_pendulum_workspace_bytes(int32_t n);
 int bte_pendulum_averages(const bte_pendulum_params* params, int32_t n, int32_t n_phase, double h, int32_t n_rk,
                           void* workspace /* device */, size_t bytes, void* cuda_stream, bte_pendulum_out* out);
 
+/* Real-space-phi_x variant of the step (BASELINE.json config 0's "64 periodic phi_x points"; NOT in the paper, whose
+ * Fourier representation (7)-(8) reduces the implicit solve to the 2x2 blocks of eq. 32-33 -- DESIGN.md C22): f is
+ * kept on n_phix periodic points phi_x_i = -pi + 2 pi i / n_phix; the Crank-Nicolson treatment of relaxation and of the
+ * (E + B phi_y) d/dphi_x term becomes ONE CYCLIC TRIDIAGONAL SYSTEM PER phi_y ROW (batched cyclic sweeps), the
+ * -B sin(phi_x) d/dphi_y term stays explicit on the staggered leap-frog grids (eq. 40-41), start-up per L202.
+ * One system per ctx; params as for bte_create (n_steps_total / avg_start_step honoured).  Same ownership rules:
+ * caller-owned DEVICE workspace of bte_rs_workspace_bytes(grid) bytes, 256-byte aligned.  bte_rs_observables fills one
+ * bte_obs (norm = sqrt(alpha) dx dphi sum f, eq. 6; v_dr = sqrt(alpha) dx dphi sum sin(phi_x) f, eq. 18-19; edge_leak 0).
+ * bte_rs_get_state: f is a HOST array of n_phix * n_phiy doubles, [i][m], m fastest; grid_id 0 whole, 1 fractional. */
+typedef struct bte_rs_ctx bte_rs_ctx;
+typedef struct {
+    int32_t n_phix;  /* periodic phi_x points, 4 .. 4096                                                   */
+    int32_t n_phiy;  /* phi_y lattice points, m = 0..M                                                      */
+    double dt;       /* time step in units of tau                                                           */
+} bte_rs_grid;
+size_t bte_rs_workspace_bytes(const bte_rs_grid* grid /* host */);
+int bte_rs_create(const bte_rs_grid* grid, const bte_params* params /* host, one entry */, void* workspace /* device */,
+                  size_t bytes, void* cuda_stream, bte_rs_ctx** out);
+int bte_rs_init_equilibrium(bte_rs_ctx* ctx);
+int bte_rs_step(bte_rs_ctx* ctx, int64_t n_steps);
+int bte_rs_observables(bte_rs_ctx* ctx, bte_obs* out /* host, one entry */);
+int bte_rs_get_state(bte_rs_ctx* ctx, int32_t grid_id, double* f /* host */);
+int bte_rs_destroy(bte_rs_ctx* ctx);
+
 /* Tuning / variant selection, before or between bte_step calls.  Keys:
  *   "variant"      0 = automatic (default), 1 = two half-update kernels per step (96 B/point/step),
  *                  2 = fused whole+fractional kernel on a 2-D tile grid (64 B/point/step),

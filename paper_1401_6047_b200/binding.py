@@ -20,7 +20,9 @@ BTE_OK, BTE_EINVAL, BTE_EUNSTABLE, BTE_ENOMEM, BTE_ECUDA = 0, -1, -2, -3, -4
 
 EXPORTS = ("bte_workspace_bytes", "bte_create", "bte_init_equilibrium", "bte_step", "bte_observables",
            "bte_destroy", "bte_get_state", "bte_set_state", "bte_reconstruct_pdf", "bte_pendulum_workspace_bytes",
-           "bte_pendulum_averages", "bte_set_option", "bte_launch_count",
+           "bte_pendulum_averages", "bte_rs_workspace_bytes", "bte_rs_create", "bte_rs_init_equilibrium",
+           "bte_rs_step", "bte_rs_observables", "bte_rs_get_state", "bte_rs_destroy", "bte_set_option",
+           "bte_launch_count",
            "bte_last_error")
 
 
@@ -33,6 +35,10 @@ class BteError(RuntimeError):
 class bte_grid(C.Structure):
     _fields_ = [("n_harm", C.c_int32), ("n_phiy", C.c_int32), ("n_batch", C.c_int32),
                 ("precision", C.c_int32), ("dt", C.c_double)]
+
+
+class bte_rs_grid(C.Structure):
+    _fields_ = [("n_phix", C.c_int32), ("n_phiy", C.c_int32), ("dt", C.c_double)]
 
 
 class bte_params(C.Structure):
@@ -94,6 +100,20 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.bte_pendulum_averages.restype = C.c_int
     lib.bte_pendulum_averages.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_double, C.c_int32, C.c_void_p,
                                           C.c_size_t, C.c_void_p, C.c_void_p]
+    lib.bte_rs_workspace_bytes.restype = C.c_size_t
+    lib.bte_rs_workspace_bytes.argtypes = [C.POINTER(bte_rs_grid)]
+    lib.bte_rs_create.restype = C.c_int
+    lib.bte_rs_create.argtypes = [C.POINTER(bte_rs_grid), C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p,
+                                  C.POINTER(C.c_void_p)]
+    for name in ("bte_rs_init_equilibrium", "bte_rs_destroy"):
+        getattr(lib, name).restype = C.c_int
+        getattr(lib, name).argtypes = [C.c_void_p]
+    lib.bte_rs_step.restype = C.c_int
+    lib.bte_rs_step.argtypes = [C.c_void_p, C.c_int64]
+    lib.bte_rs_observables.restype = C.c_int
+    lib.bte_rs_observables.argtypes = [C.c_void_p, C.POINTER(bte_obs)]
+    lib.bte_rs_get_state.restype = C.c_int
+    lib.bte_rs_get_state.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
     lib.bte_set_option.restype = C.c_int
     lib.bte_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_int64]
     lib.bte_launch_count.restype = C.c_int
@@ -143,6 +163,59 @@ def pendulum_averages(param_sets, n_phase: int = 64, h: float = 0.004, n_rk: int
 def workspace_bytes(n_harm: int, n_phiy: int, n_batch: int, dt: float) -> int:
     g = make_grid(n_harm, n_phiy, n_batch, dt)
     return int(load_library().bte_workspace_bytes(C.byref(g)))
+
+
+class RealSpaceSolver:
+    """Thin wrapper of the bte_rs_* entry points (real-space-phi_x variant: one cyclic tridiagonal Crank-Nicolson solve
+    per phi_y row; include/bte.h).  `params` is one object with the fields of bte_params."""
+
+    def __init__(self, n_phix: int, n_phiy: int, dt: float, params, device: str = "cuda:0", stream=None):
+        import torch
+        lib = load_library()
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1401_6047_b200 needs a CUDA device (B200, sm_100a); no CPU fallback")
+        self._lib = lib
+        self.grid = bte_rs_grid(int(n_phix), int(n_phiy), float(dt))
+        self.shape = (int(n_phix), int(n_phiy))
+        nbytes = int(lib.bte_rs_workspace_bytes(C.byref(self.grid)))
+        if nbytes == 0:
+            raise BteError(BTE_EINVAL, "invalid grid")
+        self.device = torch.device(device)
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            self._params = make_params([params])
+            h = C.c_void_p()
+            _check(lib.bte_rs_create(C.byref(self.grid), self._params, C.c_void_p(self.workspace.data_ptr()),
+                                     nbytes, C.c_void_p(self.stream.cuda_stream), C.byref(h)))
+            self._h = h
+
+    def init_equilibrium(self):
+        _check(self._lib.bte_rs_init_equilibrium(self._h))
+
+    def step(self, n_steps: int):
+        _check(self._lib.bte_rs_step(self._h, int(n_steps)))
+
+    def observables(self) -> "Obs":
+        o = bte_obs()
+        _check(self._lib.bte_rs_observables(self._h, C.byref(o)))
+        return Obs(*[getattr(o, f[0]) for f in bte_obs._fields_])
+
+    def get_state(self, grid_id: int):
+        f = np.empty(self.shape)
+        _check(self._lib.bte_rs_get_state(self._h, grid_id, C.c_void_p(f.ctypes.data)))
+        return f
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            self._lib.bte_rs_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
 
 
 class Solver:

@@ -514,6 +514,9 @@ extern "C" {
 
 const char* bte_last_error(void) { return g_err.c_str(); }
 
+// used by the other translation units of the library (bte_rs.cu); not declared in include/bte.h
+void bte_internal_set_error(const char* text) { g_err = text ? text : ""; }
+
 size_t bte_workspace_bytes(const bte_grid* grid) {
     if (!grid_ok(grid)) return 0;
     return offsets_for(grid).total;

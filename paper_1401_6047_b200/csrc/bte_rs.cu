@@ -1,0 +1,208 @@
+// bte_rs.cu -- host side of the real-space-phi_x variant (include/bte.h, bte_rs_* entry points).
+// Product code: must not include, link or call anything under oracle/.
+#include "../../include/bte.h"
+#include "bte_realspace.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <vector>
+
+using namespace bte;
+
+extern "C" void bte_internal_set_error(const char* text);   // bte.cu: thread-local text behind bte_last_error()
+
+namespace {
+
+int rs_fail(int code, const char* text) {
+    bte_internal_set_error(text);
+    return code;
+}
+
+#define RS_CUDA_TRY(expr)                                                                          \
+    do {                                                                                           \
+        cudaError_t e__ = (expr);                                                                  \
+        if (e__ != cudaSuccess) {                                                                  \
+            char buf__[256];                                                                       \
+            snprintf(buf__, sizeof buf__, "%s failed: %s", #expr, cudaGetErrorString(e__));        \
+            return rs_fail(BTE_ECUDA, buf__);                                                      \
+        }                                                                                          \
+    } while (0)
+
+constexpr size_t RS_ALIGN = 256;
+size_t rs_align(size_t x) { return (x + RS_ALIGN - 1) / RS_ALIGN * RS_ALIGN; }
+
+struct RsOffsets { int pitch; size_t f, cprime, zvec, ex, sinx, gm, phi, partial, obs, total; };
+
+bool rs_grid_ok(const bte_rs_grid* g) {
+    return g && g->n_phix >= 4 && g->n_phix <= 4096 && g->n_phiy >= 3 && g->dt > 0.0 && std::isfinite(g->dt);
+}
+
+RsOffsets rs_offsets(const bte_rs_grid* g) {
+    RsOffsets o{};
+    o.pitch = (g->n_phiy + 7) / 8 * 8;
+    const size_t K = (size_t)g->n_phix, p = (size_t)o.pitch, blocks = (p + 127) / 128;
+    size_t off = 0;
+    o.f = off;       off = rs_align(off + 2 * K * p * sizeof(double));
+    o.cprime = off;  off = rs_align(off + K * p * sizeof(double));
+    o.zvec = off;    off = rs_align(off + K * p * sizeof(double));
+    o.ex = off;      off = rs_align(off + K * sizeof(double));
+    o.sinx = off;    off = rs_align(off + K * sizeof(double));
+    o.gm = off;      off = rs_align(off + p * sizeof(double));
+    o.phi = off;     off = rs_align(off + p * sizeof(double));
+    o.partial = off; off = rs_align(off + blocks * 2 * sizeof(double));
+    o.obs = off;     off = rs_align(off + sizeof(RsObs));
+    o.total = off;
+    return o;
+}
+
+// I_0(x) e^{-x} by its power series / asymptotic series is overkill here: exp(mu (cos x - 1)) / (I0(mu) e^{-mu})
+// needs the scaled Bessel function only; sum the series of I0(x) e^{-x} = sum_k (x/2)^{2k} / (k!)^2 e^{-x} in
+// log space for moderate x and use the large-argument expansion beyond.
+double bessel_i0_scaled(double x) {
+    if (x < 30.0) {
+        double term = 1.0, sum = 1.0;
+        for (int k = 1; k < 500; ++k) {
+            term *= (x / 2.0) * (x / 2.0) / ((double)k * k);
+            sum += term;
+            if (term < 1e-17 * sum) break;
+        }
+        return sum * std::exp(-x);
+    }
+    double term = 1.0, sum = 1.0;                      // I0(x) e^{-x} ~ 1/sqrt(2 pi x) sum_k ((2k-1)!!)^2 / (k! (8x)^k)
+    for (int k = 1; k < 40; ++k) {
+        term *= (2.0 * k - 1.0) * (2.0 * k - 1.0) / (k * 8.0 * x);
+        if (term < 1e-17 * sum) break;
+        sum += term;
+    }
+    return sum / std::sqrt(2.0 * 3.14159265358979323846 * x);
+}
+
+}  // namespace
+
+struct bte_rs_ctx {
+    bte_rs_grid grid;
+    bte_params params;
+    RsOffsets off;
+    char* ws;
+    cudaStream_t stream;
+    RsLayout L;
+    int64_t k;          // whole-grid steps taken
+};
+
+extern "C" {
+
+size_t bte_rs_workspace_bytes(const bte_rs_grid* grid) {
+    if (!rs_grid_ok(grid)) return 0;
+    return rs_offsets(grid).total;
+}
+
+int bte_rs_create(const bte_rs_grid* grid, const bte_params* p, void* workspace, size_t bytes, void* cuda_stream,
+                  bte_rs_ctx** out) {
+    if (out) *out = nullptr;
+    if (!out || !grid || !p || !workspace) return rs_fail(BTE_EINVAL, "bte_rs_create: NULL argument");
+    if (!rs_grid_ok(grid)) return rs_fail(BTE_EINVAL, "bte_rs_create: need 4 <= n_phix <= 4096, n_phiy >= 3, dt > 0");
+    const RsOffsets off = rs_offsets(grid);
+    if (bytes < off.total) return rs_fail(BTE_ENOMEM, "bte_rs_create: workspace too small");
+    if (((uintptr_t)workspace % RS_ALIGN) != 0) return rs_fail(BTE_ENOMEM, "bte_rs_create: workspace must be 256-byte aligned");
+    const bool finite = std::isfinite(p->E_dc) && std::isfinite(p->E_omega) && std::isfinite(p->omega) &&
+                        std::isfinite(p->B) && std::isfinite(p->mu) && std::isfinite(p->alpha) &&
+                        std::isfinite(p->phiy_min) && std::isfinite(p->phiy_max) && std::isfinite(p->kappa_scale);
+    if (!finite || !(p->mu > 0.0) || !(p->alpha > 0.0) || !(p->phiy_max > p->phiy_min) || p->n_steps_total < 0 ||
+        p->avg_start_step < 0)
+        return rs_fail(BTE_EINVAL, "bte_rs_create: need finite parameters, mu > 0, alpha > 0, phiy_max > phiy_min");
+    const int K = grid->n_phix, M1 = grid->n_phiy, M = M1 - 1;
+    const double dphi = (p->phiy_max - p->phiy_min) / M;
+    if (std::fabs(p->B) * grid->dt / dphi >= 2.0)
+        return rs_fail(BTE_EUNSTABLE, "bte_rs_create: |B| dt / dphi >= 2 (scheme unstable, DESIGN.md C11)");
+    const double PI = 3.14159265358979323846;
+    const double dx = 2.0 * PI / K;
+    std::vector<double> ex(K), sx(K), gm(off.pitch, 0.0), phi(off.pitch, 0.0);
+    const double pref = (1.0 / (2.0 * PI)) * std::sqrt(p->mu / (2.0 * PI * p->alpha)) / bessel_i0_scaled(p->mu);
+    for (int i = 0; i < K; ++i) {
+        const double x = -PI + dx * i;
+        ex[i] = pref * std::exp(p->mu * (std::cos(x) - 1.0));          // eq. (13), phi_x part
+        sx[i] = std::sin(x);
+    }
+    const double centre = 0.5 * (p->phiy_min + p->phiy_max);
+    for (int m = 0; m < M1; ++m) {
+        const double ph = centre + (m - M / 2.0) * dphi;               // C8
+        double g = std::exp(-p->mu * ph * ph / 2.0);
+        if (g < 1e-300) g = 0.0;                                        // C19
+        phi[m] = ph;
+        gm[m] = g;
+    }
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    char* ws = (char*)workspace;
+    RS_CUDA_TRY(cudaMemsetAsync(ws, 0, off.total, stream));
+    RS_CUDA_TRY(cudaMemcpyAsync(ws + off.ex, ex.data(), K * sizeof(double), cudaMemcpyHostToDevice, stream));
+    RS_CUDA_TRY(cudaMemcpyAsync(ws + off.sinx, sx.data(), K * sizeof(double), cudaMemcpyHostToDevice, stream));
+    RS_CUDA_TRY(cudaMemcpyAsync(ws + off.gm, gm.data(), gm.size() * sizeof(double), cudaMemcpyHostToDevice, stream));
+    RS_CUDA_TRY(cudaMemcpyAsync(ws + off.phi, phi.data(), phi.size() * sizeof(double), cudaMemcpyHostToDevice, stream));
+    RS_CUDA_TRY(cudaStreamSynchronize(stream));
+    bte_rs_ctx* c = new bte_rs_ctx();
+    c->grid = *grid; c->params = *p; c->off = off; c->ws = ws; c->stream = stream; c->k = 0;
+    RsLayout& L = c->L;
+    L.K = K; L.M1 = M1; L.pitch = off.pitch; L.dt = grid->dt; L.dx = dx; L.dphi = dphi;
+    L.E_dc = p->E_dc; L.E_omega = p->E_omega; L.omega = p->omega; L.B = p->B; L.kappa_scale = p->kappa_scale;
+    L.norm_scale = std::sqrt(p->alpha) * dx * dphi;
+    L.f = (double*)(ws + off.f); L.cprime = (double*)(ws + off.cprime); L.zvec = (double*)(ws + off.zvec);
+    L.ex = (const double*)(ws + off.ex); L.sinx = (const double*)(ws + off.sinx);
+    L.gm = (const double*)(ws + off.gm); L.phi = (const double*)(ws + off.phi);
+    L.partial = (double*)(ws + off.partial); L.obs = (RsObs*)(ws + off.obs);
+    *out = c;
+    return BTE_OK;
+}
+
+int bte_rs_init_equilibrium(bte_rs_ctx* c) {
+    if (!c) return rs_fail(BTE_EINVAL, "bte_rs_init_equilibrium: NULL ctx");
+    const dim3 g((unsigned)((c->off.pitch + 127) / 128), (unsigned)c->grid.n_phix);
+    rs_init_kernel<<<g, 128, 0, c->stream>>>(c->L);
+    const unsigned blocks = (unsigned)((c->off.pitch + 127) / 128);
+    rs_half_update_kernel<<<blocks, 128, 0, c->stream>>>(c->L, 2, 0, 0);     // start-up z^{1/2}, L202
+    RS_CUDA_TRY(cudaGetLastError());
+    c->k = 0;
+    return BTE_OK;
+}
+
+int bte_rs_step(bte_rs_ctx* c, int64_t n_steps) {
+    if (!c) return rs_fail(BTE_EINVAL, "bte_rs_step: NULL ctx");
+    if (n_steps < 0) return rs_fail(BTE_EINVAL, "bte_rs_step: n_steps < 0");
+    const unsigned blocks = (unsigned)((c->off.pitch + 127) / 128);
+    for (int64_t s = 0; s < n_steps; ++s) {
+        if (c->params.n_steps_total > 0 && c->k >= c->params.n_steps_total) break;   // frozen
+        const int do_avg = (c->k + 1 > c->params.avg_start_step) ? 1 : 0;
+        rs_half_update_kernel<<<blocks, 128, 0, c->stream>>>(c->L, 0, (long long)c->k, do_avg);   // eq. (40)
+        rs_half_update_kernel<<<blocks, 128, 0, c->stream>>>(c->L, 1, (long long)c->k, 0);        // eq. (41), C5
+        c->k += 1;
+    }
+    RS_CUDA_TRY(cudaGetLastError());
+    return BTE_OK;
+}
+
+int bte_rs_observables(bte_rs_ctx* c, bte_obs* out) {
+    if (!c || !out) return rs_fail(BTE_EINVAL, "bte_rs_observables: NULL argument");
+    RsObs o;
+    RS_CUDA_TRY(cudaMemcpyAsync(&o, c->ws + c->off.obs, sizeof o, cudaMemcpyDeviceToHost, c->stream));
+    RS_CUDA_TRY(cudaStreamSynchronize(c->stream));
+    out->step = c->k; out->t = (double)c->k * c->grid.dt; out->norm = o.norm; out->v_dr = o.v_dr;
+    out->sum_v_dt = o.sum_v; out->sum_vcos_dt = o.sum_c; out->sum_vsin_dt = o.sum_s; out->window = o.window;
+    out->edge_leak = 0.0;
+    return BTE_OK;
+}
+
+int bte_rs_get_state(bte_rs_ctx* c, int32_t grid_id, double* f) {
+    if (!c || !f) return rs_fail(BTE_EINVAL, "bte_rs_get_state: NULL argument");
+    if (grid_id < 0 || grid_id > 1) return rs_fail(BTE_EINVAL, "bte_rs_get_state: bad grid index");
+    const size_t K = (size_t)c->grid.n_phix, M1 = (size_t)c->grid.n_phiy, p = (size_t)c->off.pitch;
+    RS_CUDA_TRY(cudaMemcpy2DAsync(f, M1 * sizeof(double), c->L.f + (size_t)grid_id * K * p, p * sizeof(double),
+                                  M1 * sizeof(double), K, cudaMemcpyDeviceToHost, c->stream));
+    RS_CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return BTE_OK;
+}
+
+int bte_rs_destroy(bte_rs_ctx* c) {
+    delete c;
+    return BTE_OK;
+}
+
+}  // extern "C"
