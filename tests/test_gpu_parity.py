@@ -174,6 +174,14 @@ def test_resident_batch_of_many_small_systems_auto():
     s.destroy()
 
 
+@pytest.mark.parametrize("N,M1", [(1, 3), (1, 4000), (300, 7), (600, 50), (3, 129), (40, 16), (97, 1025)])
+def test_odd_shapes_through_the_automatic_path(N, M1):
+    """Tall / narrow / tiny lattices through the automatic variant choice (resident CTA, cluster, grid, or sweep),
+    two bte_step calls of different lengths (>= 4 steps: resident where it fits; < 4: sweep)."""
+    w = W.small_case(N=N, M1=M1, dt=0.004, n_steps=14, avg_start=2)
+    check(w, 14, "auto", chunks=[11, 3])
+
+
 def test_resident_interleaves_with_sweep_and_budget():
     """The resident kernel and the streaming kernels share the state: alternate them; a step budget freezes
     the system exactly at n_steps_total."""
