@@ -333,7 +333,8 @@ def run_ours(args):
                    "multi_gpu": "independent replicas, one system per rank, no collective",
                    "paper_convention_updates_per_s": value * w.grid.n_harm / (w.grid.n_harm + 1)},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": recorded_traffic(w.name, steps_per_launch),
+                     "frac": achieved / peak, "frac_of_nominal_8TBs": achieved / 8000.0,
+                     "traffic": recorded_traffic(w.name, steps_per_launch),
                      "kernel": "sweep_kernel" if launches > 1 else "resident_kernel", "steps_per_launch": steps_per_launch,
                      "algorithmic_bytes_per_launch": alg_bytes,
                      "peak_source": peak_src,
@@ -343,6 +344,7 @@ def run_ours(args):
                                         "the HBM peak; 'achieved' counts what a launch really has to move"),
                      "fp64_pipe_frac": fp64_rate / fp64_peak,
                      "one_step_per_pass": (dict(one_pass, frac=one_pass["achieved_gbs"] / peak,
+                                                frac_of_nominal_8TBs=one_pass["achieved_gbs"] / 8000.0,
                                                 note="same workload, sweep_steps = 1: the HBM-bound form "
                                                      "(64 B of HBM traffic per update), measured in this run")
                                            if one_pass else None)},
