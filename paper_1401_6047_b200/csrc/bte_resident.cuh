@@ -214,8 +214,11 @@ __global__ void __launch_bounds__(1024, 1) resident_kernel(const __grid_constant
         } else {
             const unsigned sX = whole ? sH : sF, sS = whole ? sF : sH;
             const double Ea = Es[q & 63], Eb = Es[(q + 2) & 63];
-            // slab-edge columns first: their new values go to the neighbours' halo columns
-            for (int e = tid; e < nE; e += T) {
+            // slab-edge columns first: their new values go to the neighbours' halo columns.  Edge points are dealt
+            // out from the LAST compute thread downwards, interior points from thread 0 upwards: with about one
+            // point per thread no thread carries an edge point AND an interior point (the serial latency of a
+            // half-update is one point update, not two).
+            for (int e = T - 1 - tid; e < nE; e += T) {
                 const int side = e >= rows ? 1 : 0, n = e - side * rows;
                 const int j = side ? Wv - 1 : 0;
                 const double2 out = resident_point(sX, sS, n, j, PB, sph, sgdt, scn, c, L, Ea, Eb);
