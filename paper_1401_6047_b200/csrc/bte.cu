@@ -327,11 +327,13 @@ int plan_resident(bte_ctx* c) {
         else if (G <= maxg && c->grid.n_batch == 1) resident_try(c, 2, G);
         return BTE_OK;
     }
-    // automatic: the fewest slabs that leave about one point per thread (synchronisation cost grows with the
-    // number of CTAs: __syncthreads < cluster barrier < neighbour flags through L2)
-    if (pts <= 992 && resident_try(c, 0, 1)) return BTE_OK;
+    // automatic: the fewest slabs that leave at most 512 points per CTA (one point per thread, the SM's fp64 and
+    // shared-memory pipes far from saturated; measured on config 0: 3.4 / 1.9 / 1.7 us per step with 4 / 8 / 16
+    // CTAs); synchronisation cost grows with the number of CTAs: __syncthreads < cluster barrier < neighbour
+    // flags through L2
+    if (pts <= 512 && resident_try(c, 0, 1)) return BTE_OK;
     for (int G = 2; G <= 16; G *= 2)
-        if ((pts / G <= 992 || G == 16) && resident_try(c, 1, G)) return BTE_OK;
+        if ((pts / G <= 512 || G == 16) && resident_try(c, 1, G)) return BTE_OK;
     for (int G = 8; G >= 2; G /= 2)             // 16 not schedulable / does not fit: smaller clusters that fit
         if (resident_try(c, 1, G)) return BTE_OK;
     if (resident_try(c, 0, 1)) return BTE_OK;
