@@ -83,6 +83,19 @@ def test_config4_full_length():
     run_and_compare(4)
 
 
+@pytest.mark.parametrize("idx", [3, 4])
+@pytest.mark.parametrize("sweep_steps", [1, 2, 3])
+def test_streaming_configs_full_length_every_sweep_depth(idx, sweep_steps):
+    """Configs 3 (512 systems, step budgets: launches are cut at every budget boundary) and 4 at full length with
+    1, 2 and 3 time steps per pass."""
+    run_and_compare(idx, variant=3, sweep_steps=sweep_steps)
+
+
+def test_config2_full_length_streaming_kernel():
+    """Config 2 (78 540 steps) through the sweep kernel with graph replay instead of the resident kernel."""
+    run_and_compare(2, variant=3)
+
+
 @pytest.mark.parametrize("sweep_steps", [1, 2, 3])
 def test_config1_full_length_streaming_kernel(sweep_steps):
     """The same 62 832 steps through the HBM-streaming sweep kernel (graph replay) instead of the resident one."""
