@@ -182,7 +182,18 @@ def config4() -> Workload:
                    "transient to t=2; state 525 MB > L2 => HBM streaming")
 
 
-CONFIGS = {0: config0, 1: config1, 2: config2, 3: config3, 4: config4}
+def paper_table1() -> Workload:
+    """The paper's own timing run (Table 1): n-harmonics=120, g-grid=4000, dt=0.0001, t-max=10
+    (1e5 steps), E_dc=7, E_omega=0.1, omega=10, B=4, mu=116, alpha=0.9496, PhiYmin=-6, PhiYmax=6.  The paper ran it in
+    fp32 and counts MLUPS as n-harmonics x g-grid x steps / time.  Context workload (index 5), not a BASELINE config."""
+    p = Params(E_dc=7.0, E_omega=0.1, omega=10.0, B=4.0, mu=116.0, alpha=0.9496, phiy_min=-6.0, phiy_max=6.0,
+               kappa_scale=1.0, n_steps_total=0, avg_start_step=0)
+    return Workload(name="paper_table1", grid=Grid(120, 4000, 1, 1e-4), params=[p], n_steps=100000,
+                    note="the paper's Table 1 run (fp32 there): 1094 MLUPS on a GTX680, 9 MLUPS on one i7-3770 core")
+
+
+CONFIGS = {0: config0, 1: config1, 2: config2, 3: config3, 4: config4, 5: paper_table1}
+PAPER_TABLE1_MLUPS_K6 = 1094.0     # fastest CUDA kernel of the paper, GTX680, fp32 (PAPER.md:L315-321)
 
 
 def absorption_sweep(omegas, E_dc: float, E_omega: float, B: float, mu: float, N: int, M1: int, dt: float,

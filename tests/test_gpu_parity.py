@@ -309,6 +309,12 @@ def test_config3_subset_prefix():
     check(w, 200, "auto", systems=list(range(0, 512, 73)))
 
 
+def test_paper_table1_prefix():
+    """The paper's own Table 1 run (mu = 116, sharp f0; 121 x 4000 lattice), 60 steps, fp64, automatic variant."""
+    w = W.get(5)
+    check(w, 60, "auto")
+
+
 def test_config4_prefix():
     """Bandwidth-stress grid in the launch configuration bench.py times; 4 steps, full state compare."""
     w = W.config4()

@@ -77,3 +77,13 @@ def test_tucker_helper_against_the_oracle_on_cpu():
     A = absorption(sim.observables(), 50.0)
     ref = tucker_averages(50.0, 5.0, 1.0, 3.0)[2]
     assert abs(A - ref) < 2e-3 * max(abs(ref), 0.05)
+
+
+def test_paper_table1_workload_is_the_papers_command_line():
+    w = W.get(5)
+    p = w.params[0]
+    assert (w.grid.n_harm, w.grid.n_phiy, w.grid.dt, w.n_steps) == (120, 4000, 1e-4, 100000)       # L325-326
+    assert (p.E_dc, p.E_omega, p.omega, p.B, p.mu, p.alpha, p.phiy_min, p.phiy_max) == \
+        (7.0, 0.1, 10.0, 4.0, 116.0, 0.9496, -6.0, 6.0)
+    assert abs(p.B) * w.grid.dt / ((p.phiy_max - p.phiy_min) / (w.grid.n_phiy - 1)) < 1.0           # C11
+    assert abs(120 * 4000 * 1e5 / 43.85 / 1e6 - W.PAPER_TABLE1_MLUPS_K6) < 1.0                       # Table 1, K6 column
