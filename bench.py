@@ -25,7 +25,7 @@ if ROOT not in sys.path:
 
 from paper_1401_6047_b200 import workloads as W  # noqa: E402
 
-METRIC = "fp64 grid-point updates/s"
+METRIC = "fp64 grid-point updates/s per time step; achieved HBM GB/s vs B200 peak"   # BASELINE.json "metric"
 UNIT = "updates/s"
 BYTES_PER_UPDATE = 64.0   # a_h, b_h, a_f, b_f each read once and written once
 
