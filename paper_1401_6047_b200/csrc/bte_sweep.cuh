@@ -144,7 +144,9 @@ struct SweepShared {
 };
 
 // One segment: system sys, strip, rows r0 .. r0+Lr-1.
-template <int T, int S>
+// SKIP: in the fill / drain iterations do not compute stages whose row lies outside their range (a uniform branch);
+// pays off for batches of short columns, where fill / drain is a large share of a segment (used when BUDGETS).
+template <int T, int S, bool SKIP>
 __device__ __forceinline__ void sweep_segment(const Layout& L, const int sys, const int strip, const int r0,
                                               const int Lr, const int n_strips, const unsigned ups,
                                               double2* smem, SweepShared<T, S>& sh) {
@@ -268,9 +270,12 @@ __device__ __forceinline__ void sweep_segment(const Layout& L, const int sys, co
         // iterations, so they are independent of this iteration's results and can be in flight together)
         double2 d0s[NS], ws[NS];
         double cjs[NS];
+        bool act[NS];
 #pragma unroll
         for (int j = 0; j < NS; ++j) {
             const int row = row0 - 2 * j;                            // row formed by stage j
+            act[j] = true;
+            if (EDGE && SKIP) { ws[j] = zero; cjs[j] = 0.0; }
             // phi_y-difference of row+1 of the stencil grid X^j (row 0 pre-doubled in a: chi(1) = 2, eq. 11)
             {
                 unsigned a;
@@ -280,6 +285,10 @@ __device__ __forceinline__ void sweep_segment(const Layout& L, const int sys, co
                 const double2 l = lds_d2(a), r = lds_d2(a + 32);
                 d0s[j].x = __dsub_rn(r.x, l.x); d0s[j].y = __dsub_rn(r.y, l.y);
                 if (EDGE && row + 1 == 0) d0s[j].x *= 2.0;
+            }
+            if (EDGE && SKIP) {
+                act[j] = row >= max(0, r0 - (HALO - j)) && row <= min(L.N, r0 + Lr - 1 + (HALO - j));
+                if (!act[j]) continue;                               // uniform over the CTA
             }
             // own point: X^{j-1}[row][col]
             if (j == 0) ws[j] = lds_d2(tF + tH_off + o_h);
@@ -293,12 +302,15 @@ __device__ __forceinline__ void sweep_segment(const Layout& L, const int sys, co
             const int row = row0 - 2 * j;
             const double2 d0 = d0s[j], w = ws[j];
             const double cj = cjs[j];
-            double2 out = cn_point(w, d2[j], d0, nd0 - (double)(2 * j), hb[j], hb[j + 2], __dmul_rn(cj, gdt),
-                                   kappa, L.xi, L.nu, L.nu2);
-            if (EDGE) {
-                const int lo = max(0, r0 - (HALO - j)), hi = min(L.N, r0 + Lr - 1 + (HALO - j));
-                if (row < lo || row > hi) out = zero;    // outside the lattice / outside this segment's halo
-                if (row == 0) out.y = 0.0;               // b_0 == 0 (eq. 23, C3)
+            double2 out = zero;
+            if (!(EDGE && SKIP) || act[j]) {
+                out = cn_point(w, d2[j], d0, nd0 - (double)(2 * j), hb[j], hb[j + 2], __dmul_rn(cj, gdt), kappa, L.xi,
+                               L.nu, L.nu2);
+                if (EDGE) {
+                    const int lo = max(0, r0 - (HALO - j)), hi = min(L.N, r0 + Lr - 1 + (HALO - j));
+                    if (row < lo || row > hi) out = zero;    // outside the lattice / outside this segment's halo
+                    if (row == 0) out.y = 0.0;               // b_0 == 0 (eq. 23, C3)
+                }
             }
             if (j < NS - 2) sts_d2(tF + tQ_off + j * QD * SROW + q_w + 16, out);
             if (j == NS - 2) sts_d2(tF + tQ_off + (NS - 2) * QD * SROW + l_w + 16, out);
@@ -467,7 +479,7 @@ __global__ void __launch_bounds__(T, MINB) sweep_kernel(const __grid_constant__ 
         const int Lr = (int)min((long long)(rows - r0), end - pos);
         const int sys = BUDGETS ? sh.list[a - a_first] : a;
         pos += Lr;
-        sweep_segment<T, S>(L, sys, strip, r0, Lr, n_strips, ups, smem, sh);
+        sweep_segment<T, S, BUDGETS>(L, sys, strip, r0, Lr, n_strips, ups, smem, sh);
     }
 
     // ---- the last CTA of the launch advances the step counters of all systems that were active --------
