@@ -693,7 +693,14 @@ int bte_step(bte_ctx* c, int64_t n_steps) {
             c->steps_issued += glen * S;
         }
     }
+    // every system has a budget and all of them are spent: nothing left to launch
+    bool all_budgeted = c->has_budgets;
+    for (size_t i = 0; all_budgeted && i < c->params.size(); ++i) all_budgeted = c->params[i].n_steps_total > 0;
     while (left > 0) {
+        if (all_budgeted && c->steps_issued >= c->budgets.back()) {
+            c->steps_issued += left;
+            break;
+        }
         // an s-step launch must not contain a budget boundary in its interior (a system that would freeze
         // after fewer than s steps): shorten the group to end exactly on the next boundary
         int64_t s = std::min<int64_t>(S, left);
