@@ -121,7 +121,7 @@ def run_reference(args):
     from oracle import OracleSim, max_threads
     w = W.get(args.workload)
     threads = max_threads()
-    cols, p = oracle_sample(w, args.steps, args.warmup)
+    cols, p = oracle_sample(w, args.steps, args.warmup, args.ref_budget)
     sim = OracleSim(w.grid.n_harm, cols, w.grid.dt, p, threads=threads)
     sim.init_equilibrium()
     sim.step(args.warmup)
@@ -398,6 +398,8 @@ def main():
     ap.add_argument("--sweep-threads", type=int, default=0, help="threads per CTA of the sweep kernel (0 auto)")
     ap.add_argument("--res-ctas", type=int, default=0, help="slabs of the resident kernel (0 auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-budget", type=float, default=2.5e9,
+                    help="--impl reference: grid-point updates of the bounded oracle sample (steps + warmup together)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
