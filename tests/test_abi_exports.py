@@ -57,6 +57,10 @@ def test_workspace_bytes_is_a_pure_function(lib):
     assert lib.bte_workspace_bytes(C.byref(binding.make_grid(20, 201, 0, 0.005))) == 0     # n_batch < 1
     assert lib.bte_workspace_bytes(C.byref(binding.make_grid(20, 201, 1, 0.0))) == 0       # dt <= 0
     assert lib.bte_workspace_bytes(None) == 0
+    # fp32 storage (bte_grid.precision 1, 2): half the bytes per lattice point; precision outside 0..2 is invalid
+    half = lib.bte_workspace_bytes(C.byref(binding.make_grid(512, 32001, 1, 0.001, precision=2)))
+    assert 0.49 * big < half < 0.52 * big
+    assert lib.bte_workspace_bytes(C.byref(binding.make_grid(20, 201, 1, 0.005, precision=3))) == 0
 
 
 def _create(lib, grid, params, ws=0x10000, nbytes=1 << 40):
