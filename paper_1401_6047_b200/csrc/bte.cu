@@ -2,6 +2,7 @@
 // Product code: must not include, link or call anything under oracle/.
 #include "../../include/bte.h"
 #include "bte_sweep.cuh"
+#include "bte_regsweep.cuh"
 #include "bte_resident.cuh"
 #include "bte_pendulum.cuh"
 #include "bte_lowprec.cuh"
@@ -107,7 +108,7 @@ void bessel_i_ratios(double x, int N, std::vector<double>& r) {
     for (int n = 0; n <= N; ++n) r[n] = t[n] / t[0];
 }
 
-enum Variant { VAR_AUTO = 0, VAR_SPLIT = 1, VAR_FUSED = 2, VAR_SWEEP = 3, VAR_RESIDENT = 4 };
+enum Variant { VAR_AUTO = 0, VAR_SPLIT = 1, VAR_FUSED = 2, VAR_SWEEP = 3, VAR_RESIDENT = 4, VAR_REGSWEEP = 5 };
 
 }  // namespace
 
@@ -133,6 +134,8 @@ struct bte_ctx {
     int sweep_ctas;                  // option: grid-size override (0 = SMs x resident CTAs)
     int sweep_threads;               // option: 0 = automatic, 128, 256
     int sw_grid[SWEEP_MAX_STEPS + 1];   // grid of the S-step kernel; 0 = not usable for this problem
+    int rs_grid[SWEEP_MAX_STEPS + 1];   // same for the register-pipelined kernel (bte_regsweep.cuh), S >= 2
+    int rs_cols;                     // option: columns per lane of the register-pipelined kernel (0 = automatic)
     int sm_count;
     std::vector<int64_t> budgets;    // sorted distinct step budgets (n_steps_total > 0)
     // resident (on-chip) kernel launch plan
@@ -182,7 +185,7 @@ int plan_fused(bte_ctx* c) {
 // resident CTAs per SM the register budget of each instantiation is compiled for
 template <int S> struct SweepMinB { static constexpr int v = S == 1 ? 4 : S == 2 ? 3 : 2; };
 
-struct SweepFn { void* fn; size_t smem; int W; int T; };
+struct SweepFn { void* fn; size_t smem; int W; int T; int strips_per_band; };
 
 // T = 128 threads per CTA (several CTAs per SM) or T = 256 (half the strip-halo overhead, longer DRAM bursts
 // per row; S = 3 then runs one CTA per SM)
@@ -191,7 +194,7 @@ SweepFn sweep_fn_ts(bool budgets) {
     using Cfg = SweepCfg<T, S>;
     constexpr int MB = T == 128 ? SweepMinB<S>::v : (S == 1 && T == 256 ? 2 : 1);
     return {budgets ? (void*)sweep_kernel<T, S, true, MB> : (void*)sweep_kernel<T, S, false, MB>,
-            Cfg::smem_bytes, Cfg::W, T};
+            Cfg::smem_bytes, Cfg::W, T, 1};
 }
 
 SweepFn sweep_fn(int S, bool budgets, int wide) {
@@ -209,7 +212,24 @@ SweepFn sweep_fn(int S, bool budgets, int wide) {
         default: return sweep_fn_ts<128, 3>(budgets);
     }
 }
-static_assert(SWEEP_MAX_STEPS == 3, "instantiate sweep_kernel for every S up to SWEEP_MAX_STEPS");
+constexpr int RING_MAX_STEPS = 3;   // the shared-memory-ring kernel is instantiated for S = 1 .. 3
+static_assert(SWEEP_MAX_STEPS == 4, "instantiate regsweep_kernel for every S from 2 up to SWEEP_MAX_STEPS");
+
+// register-pipelined kernel (bte_regsweep.cuh): S = 2 .. SWEEP_MAX_STEPS steps per pass, K = 2 columns per lane
+constexpr int RS_K = 2;
+template <int S>
+SweepFn regsweep_fn_s(bool budgets) {
+    using Cfg = RegCfg<S, RS_K>;
+    return {budgets ? (void*)regsweep_kernel<S, RS_K, true> : (void*)regsweep_kernel<S, RS_K, false>,
+            Cfg::smem_bytes, Cfg::W, Cfg::T, Cfg::STRIPS};
+}
+SweepFn regsweep_fn(int S, bool budgets) {
+    switch (S) {
+        case 2: return regsweep_fn_s<2>(budgets);
+        case 3: return regsweep_fn_s<3>(budgets);
+        default: return regsweep_fn_s<4>(budgets);
+    }
+}
 
 // Wider CTAs pay off only for the HBM-bound one-step pass over long rows (4 or 8 KB DRAM bursts per row instead
 // of 2 KB: 74 / 79 / 81 G updates/s on config 4 with 128 / 256 / 512 threads); the multi-step passes are faster
@@ -221,14 +241,38 @@ int sweep_wide(const bte_ctx* c, int S) {
 }
 
 int plan_sweep(bte_ctx* c) {
-    for (int S = 0; S <= SWEEP_MAX_STEPS; ++S) c->sw_grid[S] = 0;
+    for (int S = 0; S <= SWEEP_MAX_STEPS; ++S) c->sw_grid[S] = c->rs_grid[S] = 0;
     if (c->grid.precision != 0) return BTE_OK;     // fp32 variants run the split kernels only
     int dev = 0, sms = 0;
     CUDA_TRY(cudaGetDevice(&dev));
     CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     c->sm_count = sms;
     const long long rows_alloc = c->grid.n_harm + 1 + 2 * GHOST;
-    for (int S = 1; S <= SWEEP_MAX_STEPS; ++S) {
+    // register-pipelined kernel: one CTA (teams of S warps) per SM; a CTA range is counted in band-rows
+    for (int S = 2; S <= SWEEP_MAX_STEPS; ++S) {
+        const SweepFn f = regsweep_fn(S, c->has_budgets);
+        int occ = 0;
+        cudaError_t e = cudaFuncSetAttribute(f.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f.smem);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f.fn, f.T, f.smem);
+        if (e != cudaSuccess)
+            return fail(BTE_ECUDA, "regsweep_kernel<S=%d> setup failed: %s (is this an sm_100a device?)", S,
+                        cudaGetErrorString(e));
+        if (occ < 1) continue;
+        const long long strips = (c->grid.n_phiy + f.W - 1) / f.W;
+        const long long bands = (strips + f.strips_per_band - 1) / f.strips_per_band;
+        const long long units = bands * (c->grid.n_harm + 1) * (long long)c->grid.n_batch;
+        if (2LL * c->grid.n_batch * rows_alloc * c->off.pitch >= (1LL << 31)) continue;   // 32-bit element offsets
+        if (S * strips * (c->grid.n_harm + 1) >= (1LL << 31) || units >= (1LL << 31)) continue;
+        long long g = (long long)sms * occ;
+        // a segment costs about NS + HALO extra row iterations: a CTA should own a few times that many rows
+        const long long min_rows = c->sweep_ctas > 0 ? 1 : 8 * S;
+        if (c->sweep_ctas > 0) g = c->sweep_ctas;
+        if (g > (units + min_rows - 1) / min_rows) g = (units + min_rows - 1) / min_rows;
+        if (g < 1) g = 1;
+        if (c->has_budgets && (long long)c->grid.n_batch / g + 2 > RegCfg<2, RS_K>::MAX_SPAN) continue;
+        c->rs_grid[S] = (int)g;
+    }
+    for (int S = 1; S <= RING_MAX_STEPS; ++S) {
         c->sw_grid[S] = 0;
         const SweepFn f = sweep_fn(S, c->has_budgets, sweep_wide(c, S));
         int occ = 0;
@@ -372,20 +416,46 @@ int launch_resident(bte_ctx* c, int64_t n_steps) {
 
 int effective_variant(const bte_ctx* c) {
     if (c->grid.precision != 0) return VAR_SPLIT;
-    if (c->variant == VAR_AUTO) return c->sw_grid[1] > 0 ? VAR_SWEEP : VAR_FUSED;
-    if ((c->variant == VAR_SWEEP || c->variant == VAR_RESIDENT) && c->sw_grid[1] == 0) return VAR_FUSED;
-    if (c->variant == VAR_RESIDENT) return VAR_SWEEP;   // what runs when the resident kernel is not used
+    if (c->variant == VAR_REGSWEEP && c->sw_grid[1] > 0 && c->rs_grid[2] > 0) return VAR_REGSWEEP;
+    // AUTO, and what runs when the resident kernel is not used: the shared-memory-ring sweep kernel
+    const bool streaming = c->variant == VAR_AUTO || c->variant == VAR_RESIDENT || c->variant == VAR_REGSWEEP;
+    if (streaming || c->variant == VAR_SWEEP) return c->sw_grid[1] > 0 ? VAR_SWEEP : VAR_FUSED;
     return c->variant;
 }
 
-// steps fused per launch by the sweep kernel (the other variants advance one step per launch group)
+bool is_sweep(int var) { return var == VAR_SWEEP || var == VAR_REGSWEEP; }
+
+// is an s-step launch available in the effective streaming variant?  (one-step launches always run the
+// shared-memory-ring kernel: the HBM-bound form, bte_sweep.cuh)
+bool sweep_has(const bte_ctx* c, int var, int s) {
+    if (s == 1) return c->sw_grid[1] > 0;
+    return var == VAR_REGSWEEP ? c->rs_grid[s] > 0 : (s <= RING_MAX_STEPS && c->sw_grid[s] > 0);
+}
+
+// steps fused per launch by the sweep kernels (the other variants advance one step per launch group)
 int sweep_steps(const bte_ctx* c) {
-    if (effective_variant(c) != VAR_SWEEP) return 1;
-    // automatic depth: 3 steps per pass when the march over n is long enough to amortise the 3 NS - 1
-    // fill/drain iterations of a segment, else 2 (measured on configs 3 and 4)
-    int S = c->sweep_steps > 0 ? c->sweep_steps : (c->grid.n_harm + 1 >= 96 ? 3 : 2);
-    while (S > 1 && c->sw_grid[S] == 0) --S;
+    const int var = effective_variant(c);
+    if (!is_sweep(var)) return 1;
+    int S;
+    if (var == VAR_REGSWEEP) {
+        S = c->sweep_steps > 0 ? c->sweep_steps : 3;
+    } else {
+        // ring kernel: 3 steps per pass when the march over n is long enough to amortise the 3 NS - 1
+        // fill/drain iterations of a segment, else 2 (measured on configs 3 and 4)
+        S = c->sweep_steps > 0 ? c->sweep_steps : (c->grid.n_harm + 1 >= 96 ? 3 : 2);
+    }
+    while (S > 1 && !sweep_has(c, var, S)) --S;
     return S;
+}
+
+// kernel, launch shape and grid of an s-step launch of the effective streaming variant
+SweepFn sweep_launch(const bte_ctx* c, int var, int s, int* grid) {
+    if (var == VAR_REGSWEEP && s >= 2) {
+        *grid = c->rs_grid[s];
+        return regsweep_fn(s, c->has_budgets);
+    }
+    *grid = c->sw_grid[s];
+    return sweep_fn(s, c->has_budgets, sweep_wide(c, s));
 }
 
 void drop_graph(bte_ctx* c) {
@@ -413,10 +483,11 @@ int launches_per_step(const bte_ctx* c) { return effective_variant(c) == VAR_SPL
 // Issue one launch group with plain launches: S steps (sweep kernel) or one step (other variants).
 int launch_steps(bte_ctx* c, int S) {
     const int var = effective_variant(c);
-    if (var == VAR_SWEEP) {
-        const SweepFn f = sweep_fn(S, c->has_budgets, sweep_wide(c, S));
+    if (is_sweep(var)) {
+        int grid = 0;
+        const SweepFn f = sweep_launch(c, var, S, &grid);
         void* args[] = {&c->L};
-        CUDA_TRY(cudaLaunchKernel(f.fn, dim3(c->sw_grid[S]), dim3(f.T), args, f.smem, c->stream));
+        CUDA_TRY(cudaLaunchKernel(f.fn, dim3(grid), dim3(f.T), args, f.smem, c->stream));
     } else if (var == VAR_FUSED) {
         fused_step_kernel<FT, FD><<<c->fgrid, FT, FCfg::smem_bytes, c->stream>>>(c->L, c->rows_per_chunk);
     } else {
@@ -460,10 +531,11 @@ int build_graph(bte_ctx* c, int64_t len, int S) {
             prev = node;
             return e;
         };
-        if (var == VAR_SWEEP) {
-            const SweepFn f = sweep_fn(S, c->has_budgets, sweep_wide(c, S));
+        if (is_sweep(var)) {
+            int grid = 0;
+            const SweepFn f = sweep_launch(c, var, S, &grid);
             void* args[] = {&c->L};
-            CUDA_TRY(add(f.fn, dim3(c->sw_grid[S]), dim3(f.T), f.smem, args));
+            CUDA_TRY(add(f.fn, dim3(grid), dim3(f.T), f.smem, args));
         } else if (var == VAR_FUSED) {
             void* args[] = {&c->L, &rpc};
             CUDA_TRY(add((void*)fused_step_kernel<FT, FD>, c->fgrid, dim3(FT), FCfg::smem_bytes, args));
@@ -612,7 +684,8 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
     c->budgets.erase(std::unique(c->budgets.begin(), c->budgets.end()), c->budgets.end());
     c->sweep_steps = 0; c->sweep_ctas = 0; c->sm_count = 0; c->graph_S = 0; c->sweep_threads = 0;
     c->res_ctas_opt = 0; c->res_mode = -1; c->res_G = 0; c->res_Wc = 0; c->res_T = 0; c->res_smem = 0;
-    for (int S = 0; S <= SWEEP_MAX_STEPS; ++S) c->sw_grid[S] = 0;
+    for (int S = 0; S <= SWEEP_MAX_STEPS; ++S) c->sw_grid[S] = c->rs_grid[S] = 0;
+    c->rs_cols = 0;
     c->steps_issued = 0; c->launches = 0;
     c->variant = VAR_AUTO; c->graph_steps = -1;
     c->tile_rows = 0;
@@ -705,6 +778,7 @@ int bte_step(bte_ctx* c, int64_t n_steps) {
         // after fewer than s steps): shorten the group to end exactly on the next boundary
         int64_t s = std::min<int64_t>(S, left);
         if (c->has_budgets) s = std::min<int64_t>(s, steps_to_next_budget(c, c->steps_issued));
+        while (s > 1 && is_sweep(var) && !sweep_has(c, var, (int)s)) --s;
         int rc = launch_steps(c, (int)s);
         if (rc != BTE_OK) return rc;
         left -= s;
@@ -854,7 +928,7 @@ int bte_pendulum_averages(const bte_pendulum_params* params, int32_t n, int32_t 
 int bte_set_option(bte_ctx* c, const char* key, int64_t value) {
     if (!c || !key) return fail(BTE_EINVAL, "bte_set_option: NULL argument");
     if (!strcmp(key, "variant")) {
-        if (value < 0 || value > 4) return fail(BTE_EINVAL, "variant must be 0, 1, 2, 3 or 4");
+        if (value < 0 || value > 5) return fail(BTE_EINVAL, "variant must be 0, 1, 2, 3, 4 or 5");
         c->variant = (int)value;
         drop_graph(c);
         return BTE_OK;

@@ -15,9 +15,10 @@ from parity_util import assert_obs_close, assert_state_close, oracle_run
 pytestmark = pytest.mark.gpu
 
 # name -> (variant, leap-frog steps fused per launch of the sweep kernel)
+# (variant 3: shared-memory-ring kernel bte_sweep.cuh; variant 5: register-pipelined kernel bte_regsweep.cuh)
 VARIANTS = {"split": (1, 0), "fused": (2, 0), "sweep1": (3, 1), "sweep2": (3, 2), "sweep3": (3, 3),
-            "resident": (4, 0), "auto": (0, 0)}
-SWEEPS = ["sweep1", "sweep2", "sweep3"]
+            "reg2": (5, 2), "reg3": (5, 3), "reg4": (5, 4), "resident": (4, 0), "auto": (0, 0)}
+SWEEPS = ["sweep1", "sweep2", "sweep3", "reg2", "reg3", "reg4"]
 ALL = ["split", "fused"] + SWEEPS + ["resident"]
 
 
