@@ -32,6 +32,8 @@
  *     batches stream through HBM once per 2-3 time steps (sweep kernel).  Results do not depend on the choice
  *     beyond rounding of the sums (the state is bit-identical across variants).
  *   - Beyond the time step: bte_reconstruct_pdf (eq. 8) and bte_pendulum_averages (eq. 44-46), see below.
+ *   - A ctx belongs to the CUDA device that owns its workspace: every entry point selects that device for the
+ *     duration of the call and restores the caller's current device.
  *   - Not thread-safe per ctx; distinct ctxs may be used from distinct threads.
  */
 #ifndef BTE_B200_H
@@ -39,6 +41,13 @@
 
 #include <stddef.h>
 #include <stdint.h>
+
+/* The library is built with -fvisibility=hidden: exactly the functions declared here are exported. */
+#if defined(__GNUC__)
+#define BTE_API __attribute__((visibility("default")))
+#else
+#define BTE_API
+#endif
 
 #ifdef __cplusplus
 extern "C" {
@@ -93,7 +102,7 @@ typedef struct {
 } bte_obs;
 
 /* Bytes of device workspace bte_create needs for this grid.  Pure function; 0 if grid is invalid. */
-size_t bte_workspace_bytes(const bte_grid* grid /* host */);
+BTE_API size_t bte_workspace_bytes(const bte_grid* grid /* host */);
 
 /* Validates, computes the per-system tables on the host (phi_y lattice, Gaussian factor, Bessel ratios
  * I_n(mu)/I_0(mu) of eq. 15) and uploads them into the workspace.
@@ -102,35 +111,41 @@ size_t bte_workspace_bytes(const bte_grid* grid /* host */);
  *                  valid until bte_destroy.  bytes is its size.
  *   cuda_stream  : cudaStream_t (as void*) on which all work of this ctx is issued.
  *   out          : host; receives the ctx, or NULL on failure.                                          */
-int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, size_t bytes,
+BTE_API int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, size_t bytes,
                void* cuda_stream, bte_ctx** out);
 
 /* State at t = 0: whole grid a = a^(0), b = 0 (L99); fractional grid by T with dt/2 (L202); step counter,
  * running sums and observables reset.  Asynchronous on the stream.                                      */
-int bte_init_equilibrium(bte_ctx* ctx);
+BTE_API int bte_init_equilibrium(bte_ctx* ctx);
 
 /* Advance every system that has not reached its n_steps_total by n_steps (>= 0) steps of eq. (40)-(41)
  * with the per-step reductions.  Asynchronous on the stream; no host synchronisation inside.            */
-int bte_step(bte_ctx* ctx, int64_t n_steps);
+BTE_API int bte_step(bte_ctx* ctx, int64_t n_steps);
 
 /* Synchronises the stream and writes grid->n_batch records to out (host). */
-int bte_observables(bte_ctx* ctx, bte_obs* out /* host, n_batch entries */);
+BTE_API int bte_observables(bte_ctx* ctx, bte_obs* out /* host, n_batch entries */);
 
 /* Frees the ctx (host object and CUDA graph handles).  Never touches the workspace memory. */
-int bte_destroy(bte_ctx* ctx);
+BTE_API int bte_destroy(bte_ctx* ctx);
 
 /* State access (tests, checkpointing, end-to-end use).  grid_id: 0 = whole grid z^k, 1 = fractional grid
  * z^{k+1/2}.  a, b: HOST arrays of (n_harm+1) * n_phiy doubles each, row-major, m fastest.  Both calls
  * synchronise the stream.  bte_set_state does not change the step counter or the running sums.          */
-int bte_get_state(bte_ctx* ctx, int32_t system, int32_t grid_id, double* a, double* b);
-int bte_set_state(bte_ctx* ctx, int32_t system, int32_t grid_id, const double* a, const double* b);
+BTE_API int bte_get_state(bte_ctx* ctx, int32_t system, int32_t grid_id, double* a, double* b);
+BTE_API int bte_set_state(bte_ctx* ctx, int32_t system, int32_t grid_id, const double* a, const double* b);
+
+/* The same for ALL systems of the batch at once: a, b are HOST arrays of n_batch * (n_harm+1) * n_phiy doubles,
+ * [system][n][m].  One launch group and ONE stream synchronisation per call, whatever n_batch is (pinned host memory
+ * makes the two copies asynchronous DMA transfers).  Afterwards every system's live ping-pong buffer is buffer 0.    */
+BTE_API int bte_get_state_batch(bte_ctx* ctx, int32_t grid_id, double* a, double* b);
+BTE_API int bte_set_state_batch(bte_ctx* ctx, int32_t grid_id, const double* a, const double* b);
 
 /* The distribution function itself, eq. (8) (L63-64): f(phi_x, phi_y_m) = sum_n a_{n,m} cos(n phi_x) + b_{n,m} sin(n phi_x)
  * of one system and grid on n_phix equidistant points phi_x_i = -pi + 2 pi i / n_phix, i = 0 .. n_phix-1 (the content
  * of the paper's Fig. 2 and Fig. 5, as a headless buffer).
  *   f : DEVICE, caller-owned, n_phix * n_phiy doubles, row-major [i][m], m fastest.  1 <= n_phix <= 2048.
  * Reads the step counter's buffer flag (synchronises the stream once), then runs asynchronously on the stream. */
-int bte_reconstruct_pdf(bte_ctx* ctx, int32_t system, int32_t grid_id, int32_t n_phix, double* f /* device */);
+BTE_API int bte_reconstruct_pdf(bte_ctx* ctx, int32_t system, int32_t grid_id, int32_t n_phix, double* f /* device */);
 
 /* The zero-temperature limit of the model, eq. (44)-(46) (L229-240): one electron starts at (phi_x, phi_y) = (0, 0) and
  * follows d phi_x/dt = E(t) + B phi_y, d phi_y/dt = -B sin(phi_x); its velocity sin(phi_x) enters the drift velocity
@@ -142,8 +157,8 @@ int bte_reconstruct_pdf(bte_ctx* ctx, int32_t system, int32_t grid_id, int32_t n
  * Independent of any ctx.  Synchronises the stream before returning.                                          */
 typedef struct { double E_dc, E_omega, omega, B; } bte_pendulum_params;
 typedef struct { double v_mean, v_cos, v_sin; } bte_pendulum_out;
-size_t bte_pendulum_workspace_bytes(int32_t n);
-int bte_pendulum_averages(const bte_pendulum_params* params, int32_t n, int32_t n_phase, double h, int32_t n_rk,
+BTE_API size_t bte_pendulum_workspace_bytes(int32_t n);
+BTE_API int bte_pendulum_averages(const bte_pendulum_params* params, int32_t n, int32_t n_phase, double h, int32_t n_rk,
                           void* workspace /* device */, size_t bytes, void* cuda_stream, bte_pendulum_out* out);
 
 /* Real-space-phi_x variant of the step (BASELINE.json config 0's "64 periodic phi_x points"; NOT in the paper, whose
@@ -161,39 +176,50 @@ typedef struct {
     int32_t n_phiy;  /* phi_y lattice points, m = 0..M                                                      */
     double dt;       /* time step in units of tau                                                           */
 } bte_rs_grid;
-size_t bte_rs_workspace_bytes(const bte_rs_grid* grid /* host */);
-int bte_rs_create(const bte_rs_grid* grid, const bte_params* params /* host, one entry */, void* workspace /* device */,
+BTE_API size_t bte_rs_workspace_bytes(const bte_rs_grid* grid /* host */);
+BTE_API int bte_rs_create(const bte_rs_grid* grid, const bte_params* params /* host, one entry */, void* workspace /* device */,
                   size_t bytes, void* cuda_stream, bte_rs_ctx** out);
-int bte_rs_init_equilibrium(bte_rs_ctx* ctx);
-int bte_rs_step(bte_rs_ctx* ctx, int64_t n_steps);
-int bte_rs_observables(bte_rs_ctx* ctx, bte_obs* out /* host, one entry */);
-int bte_rs_get_state(bte_rs_ctx* ctx, int32_t grid_id, double* f /* host */);
-int bte_rs_destroy(bte_rs_ctx* ctx);
+BTE_API int bte_rs_init_equilibrium(bte_rs_ctx* ctx);
+BTE_API int bte_rs_step(bte_rs_ctx* ctx, int64_t n_steps);
+BTE_API int bte_rs_observables(bte_rs_ctx* ctx, bte_obs* out /* host, one entry */);
+BTE_API int bte_rs_get_state(bte_rs_ctx* ctx, int32_t grid_id, double* f /* host */);
+BTE_API int bte_rs_destroy(bte_rs_ctx* ctx);
 
 /* Tuning / variant selection, before or between bte_step calls.  Keys:
  *   "variant"      0 = automatic (default), 1 = two half-update kernels per step (96 B/point/step),
  *                  2 = fused whole+fractional kernel on a 2-D tile grid (64 B/point/step),
  *                  3 = persistent sweep kernel, S steps per launch (64/S B/point/step; the default path
- *                      for lattices larger than the GPU's shared memory),
+ *                      for lattices larger than the GPU's shared memory; intermediate time levels in shared-memory
+ *                      rings, one thread per phi_y column),
+ *                  5 = register-pipelined sweep kernel, S = 2..4 steps per launch (same traffic; one warp per
+ *                      leap-frog step, rows handed from warp to warp through per-lane shared-memory FIFOs, input rows
+ *                      by TMA bulk copies; one-step launches fall back to variant 3),
  *                  4 = resident kernel: the whole time loop of one bte_step call in ONE launch, state held
  *                      in shared memory (one system: both grids must fit the shared memory of the GPU; a batch:
  *                      each system must fit one cluster of 16 CTAs; otherwise variant 3 runs).  Automatic
  *                      choice: 4 when usable, n_steps >= 4 and (for a batch) systems of at most 8192 points.
  *   "resident_ctas" slabs (CTAs) of variant 4: 1 = one CTA, 2..16 = one thread-block cluster, more = cooperative
  *                  grid; 0 = automatic
- *   "sweep_steps"  S of variant 3: 1..3, 0 = automatic
+ *   "sweep_steps"  S of variant 3 (1..3) or 5 (2..4), 0 = automatic
  *   "sweep_ctas"   CTAs of the persistent sweep kernel, 0 = SMs x resident CTAs
  *   "sweep_threads" threads per CTA of the sweep kernel: 128, 256 or (one-step pass only) 512, 0 = automatic
  *   "graph_steps"  launches captured per CUDA graph for launch-bound grids; 0 = plain launches, -1 = auto
  *   "tile_rows"    rows per tile of variant 2 (0 = automatic)
  * Returns BTE_EINVAL for an unknown key or an unsupported value.                                        */
-int bte_set_option(bte_ctx* ctx, const char* key, int64_t value);
+BTE_API int bte_set_option(bte_ctx* ctx, const char* key, int64_t value);
+
+/* What the library would run with the current options (so that a caller can label a measurement without guessing).
+ * Keys: "effective_variant" (1, 2, 3 or 5: the streaming kernel bte_step uses when the resident kernel does not
+ * apply), "effective_sweep_steps" (leap-frog steps per launch of that kernel), "resident_usable" (1 if bte_step
+ * calls of >= 4 steps run the resident kernel in automatic mode), "resident_ctas", "variant", "device" (ordinal of
+ * the device that owns the workspace; every entry point selects it and restores the caller's device).           */
+BTE_API int bte_get_option(bte_ctx* ctx, const char* key, int64_t* out /* host */);
 
 /* Number of kernel launches (graph nodes counted individually) issued by this ctx so far. */
-int bte_launch_count(bte_ctx* ctx, int64_t* out /* host */);
+BTE_API int bte_launch_count(bte_ctx* ctx, int64_t* out /* host */);
 
 /* Thread-local text of the last error returned on this thread ("" if none). */
-const char* bte_last_error(void);
+BTE_API const char* bte_last_error(void);
 
 #ifdef __cplusplus
 }

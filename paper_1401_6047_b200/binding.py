@@ -19,7 +19,8 @@ LIB_PATH = os.path.join(_HERE, "libbte_b200.so")
 BTE_OK, BTE_EINVAL, BTE_EUNSTABLE, BTE_ENOMEM, BTE_ECUDA = 0, -1, -2, -3, -4
 
 EXPORTS = ("bte_workspace_bytes", "bte_create", "bte_init_equilibrium", "bte_step", "bte_observables",
-           "bte_destroy", "bte_get_state", "bte_set_state", "bte_reconstruct_pdf", "bte_pendulum_workspace_bytes",
+           "bte_destroy", "bte_get_state", "bte_set_state", "bte_get_state_batch", "bte_set_state_batch", "bte_get_option",
+           "bte_reconstruct_pdf", "bte_pendulum_workspace_bytes",
            "bte_pendulum_averages", "bte_rs_workspace_bytes", "bte_rs_create", "bte_rs_init_equilibrium",
            "bte_rs_step", "bte_rs_observables", "bte_rs_get_state", "bte_rs_destroy", "bte_set_option",
            "bte_launch_count",
@@ -93,6 +94,11 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.bte_get_state.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
     lib.bte_set_state.restype = C.c_int
     lib.bte_set_state.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
+    for name in ("bte_get_state_batch", "bte_set_state_batch"):
+        getattr(lib, name).restype = C.c_int
+        getattr(lib, name).argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+    lib.bte_get_option.restype = C.c_int
+    lib.bte_get_option.argtypes = [C.c_void_p, C.c_char_p, C.POINTER(C.c_int64)]
     lib.bte_reconstruct_pdf.restype = C.c_int
     lib.bte_reconstruct_pdf.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p]
     lib.bte_pendulum_workspace_bytes.restype = C.c_size_t
@@ -301,8 +307,29 @@ class Solver:
         _check(self._lib.bte_reconstruct_pdf(self._h, system, grid_id, n_phix, C.c_void_p(f.data_ptr())))
         return f
 
+    def get_state_batch(self, grid_id: int, out_a=None, out_b=None):
+        """(a, b) of ALL systems: arrays of shape (n_batch, n_harm+1, n_phiy); one synchronisation."""
+        shape = (self.n_batch,) + self.shape
+        a = np.empty(shape) if out_a is None else out_a
+        b = np.empty(shape) if out_b is None else out_b
+        assert a.shape == shape and b.shape == shape and a.flags.c_contiguous and b.flags.c_contiguous
+        _check(self._lib.bte_get_state_batch(self._h, grid_id, C.c_void_p(a.ctypes.data), C.c_void_p(b.ctypes.data)))
+        return a, b
+
+    def set_state_batch(self, grid_id: int, a, b):
+        shape = (self.n_batch,) + self.shape
+        a = np.ascontiguousarray(a, dtype=np.float64)
+        b = np.ascontiguousarray(b, dtype=np.float64)
+        assert a.shape == shape and b.shape == shape
+        _check(self._lib.bte_set_state_batch(self._h, grid_id, C.c_void_p(a.ctypes.data), C.c_void_p(b.ctypes.data)))
+
     def set_option(self, key: str, value: int):
         _check(self._lib.bte_set_option(self._h, key.encode(), int(value)))
+
+    def get_option(self, key: str) -> int:
+        v = C.c_int64()
+        _check(self._lib.bte_get_option(self._h, key.encode(), C.byref(v)))
+        return int(v.value)
 
     def launch_count(self) -> int:
         n = C.c_int64()

@@ -1,6 +1,7 @@
 // bte.cu -- host side of libbte_b200: the C ABI of include/bte.h.
 // Product code: must not include, link or call anything under oracle/.
 #include "../../include/bte.h"
+#include "bte_internal.h"
 #include "bte_sweep.cuh"
 #include "bte_regsweep.cuh"
 #include "bte_resident.cuh"
@@ -20,6 +21,25 @@ using namespace bte;
 namespace {
 
 thread_local std::string g_err;
+
+// Every entry point runs on the device that owns the ctx's workspace, whatever device is current in the
+// calling thread, and restores the caller's device on return.
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev) {
+        int cur = -1;
+        if (cudaGetDevice(&cur) != cudaSuccess) { ok = false; return; }
+        if (cur != dev) {
+            if (cudaSetDevice(dev) != cudaSuccess) { ok = false; return; }
+            prev = cur;
+        }
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define CTX_GUARD(c)                                                                                \
+    DeviceGuard guard__((c)->device);                                                               \
+    if (!guard__.ok) return fail(BTE_ECUDA, "cannot select CUDA device %d of this ctx", (c)->device)
 
 int fail(int code, const char* fmt, ...) {
     char buf[512];
@@ -117,6 +137,7 @@ struct bte_ctx {
     std::vector<bte_params> params;
     Offsets off;
     char* ws;
+    int device;             // ordinal of the device that owns the workspace
     cudaStream_t stream;
     Layout L;
     int64_t steps_issued;   // global step count requested so far (per-system count = min(this, budget))
@@ -584,12 +605,13 @@ int live_buffer(bte_ctx* c, int sys, int* buf) {
 
 }  // namespace
 
+// shared with the other translation units of the library (bte_internal.h); hidden visibility
+void bte_internal_set_error(const char* text) { g_err = text ? text : ""; }
+
 extern "C" {
 
 const char* bte_last_error(void) { return g_err.c_str(); }
 
-// used by the other translation units of the library (bte_rs.cu); not declared in include/bte.h
-void bte_internal_set_error(const char* text) { g_err = text ? text : ""; }
 
 size_t bte_workspace_bytes(const bte_grid* grid) {
     if (!grid_ok(grid)) return 0;
@@ -622,6 +644,18 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
                         std::fabs(p.B) * grid->dt / dphi);
     }
     cudaStream_t stream = (cudaStream_t)cuda_stream;
+    // the device that owns the workspace is the device of this ctx (first CUDA call: after all argument checks)
+    int device = 0;
+    {
+        cudaPointerAttributes attr{};
+        if (cudaPointerGetAttributes(&attr, workspace) != cudaSuccess || attr.type != cudaMemoryTypeDevice) {
+            cudaGetLastError();
+            return fail(BTE_EINVAL, "bte_create: workspace is not a device pointer");
+        }
+        device = attr.device;
+    }
+    DeviceGuard guard__(device);
+    if (!guard__.ok) return fail(BTE_ECUDA, "bte_create: cannot select CUDA device %d", device);
 
     // host tables: phi_y lattice (C8), Gaussian factor and c_n of eq. (15)-(16) (C1, C13)
     const size_t rows = (size_t)N + 1 + 2 * GHOST, pitch = (size_t)off.pitch;   // with ghost entries (zero)
@@ -664,7 +698,7 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
     bte_ctx* c = new bte_ctx();
     c->grid = *grid;
     c->params.assign(params, params + nb);
-    c->off = off; c->ws = ws; c->stream = stream;
+    c->off = off; c->ws = ws; c->stream = stream; c->device = device;
     c->L.N = N; c->L.M1 = M1; c->L.pitch = off.pitch; c->L.n_batch = nb; c->L.dt = grid->dt;
     c->L.nu = 1.0 + 0.5 * grid->dt; c->L.xi = 1.0 - 0.5 * grid->dt; c->L.nu2 = c->L.nu * c->L.nu;
     c->L.hd = 0.5 * grid->dt;
@@ -708,6 +742,7 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
 
 int bte_init_equilibrium(bte_ctx* c) {
     if (!c) return fail(BTE_EINVAL, "bte_init_equilibrium: NULL ctx");
+    CTX_GUARD(c);
     const dim3 g((unsigned)((c->off.pitch + 127) / 128), (unsigned)(c->grid.n_harm + 1), (unsigned)c->grid.n_batch);
     if (c->grid.precision == 0) {
         init_state_kernel<<<g, 128, 0, c->stream>>>(c->L);
@@ -728,6 +763,7 @@ int bte_init_equilibrium(bte_ctx* c) {
 int bte_step(bte_ctx* c, int64_t n_steps) {
     if (!c) return fail(BTE_EINVAL, "bte_step: NULL ctx");
     if (n_steps < 0) return fail(BTE_EINVAL, "bte_step: n_steps < 0");
+    CTX_GUARD(c);
     int64_t left = n_steps;
     // lattices that fit on chip: ONE launch runs the whole time loop out of shared memory (automatic choice
     // from 4 steps on -- below that the load/store of the state is not amortised)
@@ -789,6 +825,7 @@ int bte_step(bte_ctx* c, int64_t n_steps) {
 
 int bte_observables(bte_ctx* c, bte_obs* out) {
     if (!c || !out) return fail(BTE_EINVAL, "bte_observables: NULL argument");
+    CTX_GUARD(c);
     std::vector<SysState> ss((size_t)c->grid.n_batch);
     CUDA_TRY(cudaMemcpyAsync(ss.data(), c->ws + c->off.ss, ss.size() * sizeof(SysState), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(cudaStreamSynchronize(c->stream));
@@ -803,6 +840,7 @@ int bte_observables(bte_ctx* c, bte_obs* out) {
 
 int bte_destroy(bte_ctx* c) {
     if (!c) return BTE_OK;
+    DeviceGuard guard__(c->device);
     drop_graph(c);
     delete c;
     return BTE_OK;
@@ -818,6 +856,7 @@ int bte_get_state(bte_ctx* c, int32_t system, int32_t grid_id, double* a, double
     if (!c || !a || !b) return fail(BTE_EINVAL, "bte_get_state: NULL argument");
     if (system < 0 || system >= c->grid.n_batch || grid_id < 0 || grid_id > 1)
         return fail(BTE_EINVAL, "bte_get_state: bad system or grid index");
+    CTX_GUARD(c);
     const int rows = c->grid.n_harm + 1, M1 = c->grid.n_phiy, pitch = c->off.pitch;
     int buf = 0;
     { const int rc = live_buffer(c, system, &buf); if (rc != BTE_OK) return rc; }
@@ -848,6 +887,7 @@ int bte_set_state(bte_ctx* c, int32_t system, int32_t grid_id, const double* a, 
     if (!c || !a || !b) return fail(BTE_EINVAL, "bte_set_state: NULL argument");
     if (system < 0 || system >= c->grid.n_batch || grid_id < 0 || grid_id > 1)
         return fail(BTE_EINVAL, "bte_set_state: bad system or grid index");
+    CTX_GUARD(c);
     const int rows = c->grid.n_harm + 1, M1 = c->grid.n_phiy, pitch = c->off.pitch;
     int buf = 0;
     { const int rc = live_buffer(c, system, &buf); if (rc != BTE_OK) return rc; }
@@ -879,12 +919,101 @@ int bte_set_state(bte_ctx* c, int32_t system, int32_t grid_id, const double* a, 
     return BTE_OK;
 }
 
+// ---- state exchange for the whole batch (one launch group, one synchronisation) -----------------------------
+namespace {
+// every system's live state into buffer 0 (systems whose flag says 1 are copied, then the flags are cleared), so
+// that the host knows where everything is without reading the flags back
+int normalise_buffers(bte_ctx* c) {
+    const size_t per = (size_t)(c->grid.n_harm + 1 + 2 * GHOST) * c->off.pitch;
+    const dim3 g((unsigned)std::min<size_t>((per + 255) / 256, 4096), 2, (unsigned)c->grid.n_batch);
+    if (c->grid.precision == 0) copy_live_to_buffer0_kernel<double2><<<g, 256, 0, c->stream>>>(c->L);
+    else copy_live_to_buffer0_kernel<float2><<<g, 256, 0, c->stream>>>(c->L);
+    clear_buffer_flags_kernel<<<(c->grid.n_batch + 255) / 256, 256, 0, c->stream>>>(c->L);
+    CUDA_TRY(cudaGetLastError());
+    c->launches += 2;
+    return BTE_OK;
+}
+}  // namespace
+
+int bte_get_state_batch(bte_ctx* c, int32_t grid_id, double* a, double* b) {
+    if (!c || !a || !b) return fail(BTE_EINVAL, "bte_get_state_batch: NULL argument");
+    if (grid_id < 0 || grid_id > 1) return fail(BTE_EINVAL, "bte_get_state_batch: bad grid index");
+    CTX_GUARD(c);
+    const int rows = c->grid.n_harm + 1, M1 = c->grid.n_phiy, nb = c->grid.n_batch;
+    const size_t cnt = (size_t)rows * M1;
+    if (c->grid.precision != 0) {                      // fp32 storage: system by system (reference-grade variants)
+        for (int s = 0; s < nb; ++s) {
+            const int rc = bte_get_state(c, s, grid_id, a + (size_t)s * cnt, b + (size_t)s * cnt);
+            if (rc != BTE_OK) return rc;
+        }
+        return BTE_OK;
+    }
+    { const int rc = normalise_buffers(c); if (rc != BTE_OK) return rc; }
+    // de-interleave every system from buffer 0 into its own rows 0..N of buffer 1 (dead between steps)
+    const dim3 g((unsigned)((M1 + 255) / 256), (unsigned)rows, (unsigned)nb);
+    deinterleave_batch_kernel<<<g, 256, 0, c->stream>>>(c->L, grid_id);
+    CUDA_TRY(cudaGetLastError());
+    c->launches += 1;
+    const size_t gp = (size_t)(rows + 2 * GHOST) * c->off.pitch * sizeof(double2);   // bytes between systems
+    const double* stage = (const double*)(c->L.state + state_offset(c, 1, grid_id, 0));
+    CUDA_TRY(cudaMemcpy2DAsync(a, cnt * sizeof(double), stage, gp, cnt * sizeof(double), (size_t)nb,
+                               cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaMemcpy2DAsync(b, cnt * sizeof(double), stage + cnt, gp, cnt * sizeof(double), (size_t)nb,
+                               cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return BTE_OK;
+}
+
+int bte_set_state_batch(bte_ctx* c, int32_t grid_id, const double* a, const double* b) {
+    if (!c || !a || !b) return fail(BTE_EINVAL, "bte_set_state_batch: NULL argument");
+    if (grid_id < 0 || grid_id > 1) return fail(BTE_EINVAL, "bte_set_state_batch: bad grid index");
+    CTX_GUARD(c);
+    const int rows = c->grid.n_harm + 1, M1 = c->grid.n_phiy, nb = c->grid.n_batch;
+    const size_t cnt = (size_t)rows * M1;
+    if (c->grid.precision != 0) {
+        for (int s = 0; s < nb; ++s) {
+            const int rc = bte_set_state(c, s, grid_id, a + (size_t)s * cnt, b + (size_t)s * cnt);
+            if (rc != BTE_OK) return rc;
+        }
+        return BTE_OK;
+    }
+    { const int rc = normalise_buffers(c); if (rc != BTE_OK) return rc; }
+    const size_t gp = (size_t)(rows + 2 * GHOST) * c->off.pitch * sizeof(double2);
+    double* stage = (double*)(c->L.state + state_offset(c, 1, grid_id, 0));
+    CUDA_TRY(cudaMemcpy2DAsync(stage, gp, a, cnt * sizeof(double), cnt * sizeof(double), (size_t)nb,
+                               cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(cudaMemcpy2DAsync(stage + cnt, gp, b, cnt * sizeof(double), cnt * sizeof(double), (size_t)nb,
+                               cudaMemcpyHostToDevice, c->stream));
+    const dim3 g((unsigned)((c->off.pitch + 255) / 256), (unsigned)rows, (unsigned)nb);
+    interleave_batch_kernel<<<g, 256, 0, c->stream>>>(c->L, grid_id);
+    c->launches += 1;
+    if (grid_id == 0) {   // keep norm / v_dr of the observables consistent with the new whole grids
+        reduce_finalize_kernel<double2><<<reduce_grid(c), 256, 0, c->stream>>>(c->L, 0);
+        c->launches += 1;
+    }
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return BTE_OK;
+}
+
+int bte_get_option(bte_ctx* c, const char* key, int64_t* out) {
+    if (!c || !key || !out) return fail(BTE_EINVAL, "bte_get_option: NULL argument");
+    if (!strcmp(key, "effective_variant")) { *out = effective_variant(c); return BTE_OK; }
+    if (!strcmp(key, "effective_sweep_steps")) { *out = sweep_steps(c); return BTE_OK; }
+    if (!strcmp(key, "resident_usable")) { *out = c->res_mode >= 0 ? 1 : 0; return BTE_OK; }
+    if (!strcmp(key, "resident_ctas")) { *out = c->res_mode >= 0 ? c->res_G : 0; return BTE_OK; }
+    if (!strcmp(key, "device")) { *out = c->device; return BTE_OK; }
+    if (!strcmp(key, "variant")) { *out = c->variant; return BTE_OK; }
+    return fail(BTE_EINVAL, "bte_get_option: unknown key '%s'", key);
+}
+
 int bte_reconstruct_pdf(bte_ctx* c, int32_t system, int32_t grid_id, int32_t n_phix, double* f) {
     if (!c || !f) return fail(BTE_EINVAL, "bte_reconstruct_pdf: NULL argument");
     if (system < 0 || system >= c->grid.n_batch || grid_id < 0 || grid_id > 1)
         return fail(BTE_EINVAL, "bte_reconstruct_pdf: bad system or grid index");
     if (n_phix < 1 || n_phix > 2048) return fail(BTE_EINVAL, "bte_reconstruct_pdf: n_phix must be in [1, 2048]");
     if (c->grid.precision != 0) return fail(BTE_EINVAL, "bte_reconstruct_pdf: fp64 contexts only");
+    CTX_GUARD(c);
     const int rows = c->grid.n_harm + 1, M1 = c->grid.n_phiy, pitch = c->off.pitch;
     int buf = 0;
     { const int rc = live_buffer(c, system, &buf); if (rc != BTE_OK) return rc; }
@@ -927,6 +1056,7 @@ int bte_pendulum_averages(const bte_pendulum_params* params, int32_t n, int32_t 
 
 int bte_set_option(bte_ctx* c, const char* key, int64_t value) {
     if (!c || !key) return fail(BTE_EINVAL, "bte_set_option: NULL argument");
+    CTX_GUARD(c);
     if (!strcmp(key, "variant")) {
         if (value < 0 || value > 5) return fail(BTE_EINVAL, "variant must be 0, 1, 2, 3, 4 or 5");
         c->variant = (int)value;

@@ -409,6 +409,46 @@ __global__ void interleave_kernel(double2* __restrict__ z, const double* __restr
     z[(size_t)n * pitch + m] = w;
 }
 
+// ---- whole-batch forms (bte_get_state_batch / bte_set_state_batch): no host round trip for the buffer flags ------
+// Systems whose live buffer is 1 are copied into buffer 0 (both grids, ghost rows and pad columns included) ...
+template <class E2>
+__global__ void copy_live_to_buffer0_kernel(Layout L) {
+    const int sys = blockIdx.z, grid = blockIdx.y;
+    if (L.ss[sys].buf == 0) return;
+    const size_t per = grid_points(L);
+    const E2* src = (const E2*)L.state + ((size_t)(2 + grid) * L.n_batch + sys) * per;
+    E2* dst = (E2*)L.state + ((size_t)grid * L.n_batch + sys) * per;
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < per; e += (size_t)gridDim.x * blockDim.x) dst[e] = src[e];
+}
+// ... and then every flag says 0.
+__global__ void clear_buffer_flags_kernel(Layout L) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < L.n_batch) L.ss[s].buf = 0;
+}
+// buffer 0 -> de-interleaved a | b in rows 0..N of the same system and grid of buffer 1 (dead between steps)
+__global__ void deinterleave_batch_kernel(Layout L, int grid) {
+    const int sys = blockIdx.z, n = blockIdx.y, m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= L.M1) return;
+    const size_t cnt = (size_t)(L.N + 1) * L.M1;
+    const double2 w = state_ptr(L, 0, grid, sys)[(size_t)n * L.pitch + m];
+    double* stage = (double*)state_ptr(L, 1, grid, sys);
+    stage[(size_t)n * L.M1 + m] = w.x;
+    stage[cnt + (size_t)n * L.M1 + m] = w.y;
+}
+// a | b staged in buffer 1 -> interleaved state in buffer 0 (pad columns zero, b_0 = 0)
+__global__ void interleave_batch_kernel(Layout L, int grid) {
+    const int sys = blockIdx.z, n = blockIdx.y, m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= L.pitch) return;
+    const size_t cnt = (size_t)(L.N + 1) * L.M1;
+    const double* stage = (const double*)state_ptr(L, 1, grid, sys);
+    double2 w = make_double2(0.0, 0.0);
+    if (m < L.M1) {
+        w.x = stage[(size_t)n * L.M1 + m];
+        w.y = (n == 0) ? 0.0 : stage[cnt + (size_t)n * L.M1 + m];   // b_0 == 0, eq. (23)
+    }
+    state_ptr(L, 0, grid, sys)[(size_t)n * L.pitch + m] = w;
+}
+
 // ------------------------------------------------------------------------------------------------
 // the distribution function itself: f(phi_x, phi_y) = sum_n a_n cos(n phi_x) + b_n sin(n phi_x)
 // (eq. 8) on K equidistant phi_x_i = -pi + 2 pi i / K, for every phi_y lattice point; f is [K][M1], m fastest.

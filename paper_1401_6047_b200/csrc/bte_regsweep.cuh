@@ -57,11 +57,17 @@ struct RegCfg {
     static constexpr int DIN = 8;               // slots of the HBM input ring of role 0
     static constexpr int DPRE = 6;              // rows prefetched ahead (slot of record t + DPRE was read 2 iterations ago)
     static constexpr int DF = 4;                // slots of a FIFO between consecutive roles
-    static constexpr int REC = 2 * K * 32 + 2;  // double2 per record: A[K][32], B[K][32], F^0 extra columns of lanes 0, 31
+    static constexpr int REC = 2 * K * 32 + 2;  // double2 per record.  FIFO: A[K][32], B[K][32] (+2 unused); HBM input ring
+                                                // of role 0: A = COLS columns, B = COLS + 2 columns, natural column order
     static constexpr int TEAM_D2 = (DIN + (S - 1) * DF) * REC;     // double2 per team
     static constexpr int TEAM_FLAGS = (S - 1) * 2 * 32;            // u32 per team: produced[32], consumed[32] per FIFO
     static constexpr int MAX_SPAN = 64;         // distinct systems one CTA range may touch
-    static constexpr size_t smem_bytes = (size_t)STRIPS * (TEAM_D2 * 16 + TEAM_FLAGS * 4) + (size_t)WARPS * 2 * 32 * 8;
+    // shared memory: rings of all teams | counters of all teams | mbarriers of the input rings (DIN per team) | per-warp
+    // reduction slots
+    static constexpr size_t off_flags = (size_t)STRIPS * TEAM_D2 * 16;
+    static constexpr size_t off_bars = off_flags + (size_t)STRIPS * TEAM_FLAGS * 4;
+    static constexpr size_t off_accs = off_bars + (size_t)STRIPS * DIN * 8;
+    static constexpr size_t smem_bytes = off_accs + (size_t)WARPS * 2 * 32 * 8;
     static_assert(W >= 8, "strip too narrow");
     static_assert((DIN & (DIN - 1)) == 0 && (DF & (DF - 1)) == 0 && DPRE + 2 <= DIN, "ring sizes");
 };
@@ -103,24 +109,34 @@ __device__ __forceinline__ double2 lds_d2_volatile(unsigned addr) {
 __device__ __forceinline__ void sts_d2_volatile(unsigned addr, double2 v) {
     asm volatile("st.volatile.shared.v2.f64 [%0], {%1, %2};\n" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory");
 }
-__device__ __forceinline__ void cp_async16_ca_sz(unsigned smem_addr, const void* gmem_src, int src_bytes) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 16, %2;\n" ::"r"(smem_addr), "l"(gmem_src),
-                 "r"(src_bytes)
-                 : "memory");
+// ---- 1-D bulk copies (TMA engine, SASS UBLKCP) with mbarrier completion: the HBM input ring of role 0 ----
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
 }
-__device__ __forceinline__ void cp_async16_ca_sz_if(unsigned smem_addr, const void* gmem_src, int src_bytes,
-                                                    int pred) {
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(unsigned bar, unsigned parity) {
+    unsigned ok;
     asm volatile(
-        "{\n .reg .pred p;\n setp.ne.s32 p, %3, 0;\n"
-        " @p cp.async.ca.shared.global [%0], [%1], 16, %2;\n}\n" ::"r"(smem_addr),
-        "l"(gmem_src), "r"(src_bytes), "r"(pred)
+        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
         : "memory");
+    return ok != 0;
+}
+// global -> shared, `bytes` a multiple of 16, both addresses 16-byte aligned; completion is signalled on `bar`
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
 }
 
 // What one warp keeps about its place in the team's pipeline for the whole launch.
 struct RegChan {
-    unsigned in_ring;      // shared address of the ring this role reads (role 0: HBM input ring, DIN slots), this lane
+    unsigned in_ring;      // shared address of the ring this role reads (role 0: HBM input ring, DIN slots)
     unsigned out_ring;     // shared address of the FIFO this role writes (roles < S-1), this lane
+    unsigned in_bars;      // role 0: shared address of the DIN mbarriers of the input ring
     unsigned in_flags;     // shared address of this lane's produced / consumed counters of the input FIFO (+0 / +128)
     unsigned out_flags;    // ... of the output FIFO
     unsigned t_in;         // records taken so far in this launch
@@ -192,34 +208,36 @@ __device__ __forceinline__ void regsweep_segment(const Layout& L, const int sys,
     const int rho_s1 = min(min(hi0 - 2 + j0, hi1 + j0), rho_end);
 
     // ---- role 0: HBM -> input ring ---------------------------------------------------------------------
-    // record rho = (A = H^0 row rho + 2, B = F^0 row rho + 1, F^0 one column beyond the strip for lanes 0 / 31)
-    const double2* __restrict__ Hin = state_ptr(L, cur, 0, sys);   // row 0, column 0 (always a valid address)
+    // record rho = (A = H^0 row rho + 2, columns c0 - HALO .. + COLS - 1;  B = F^0 row rho + 1, one column more on
+    // each side), natural column order.  Lane 0 issues two bulk copies per record (TMA engine) DPRE records ahead;
+    // completion arrives on the slot's mbarrier.  Columns outside [0, pitch) are not copied: those parts of the ring
+    // are zeroed once per segment (boundary condition (22)-(23) in m; the pad columns M+1 .. pitch-1 are zero in HBM).
+    // Rows outside the lattice / the segment's trapezoid are not copied either: the record reads as zero.
+    const double2* __restrict__ Hin = state_ptr(L, cur, 0, sys);   // row 0, column 0
     const int rf_max = min(N, hi_base + 1), rh_max = min(N, hi_base);      // last F^0 / H^0 row needed
-    const int xoff = (lane == 0) ? -1 : K;              // extra column relative to col0
-    const int xlane = (lane == 0 || lane == 31) ? 1 : 0;
-    const bool xvalid = xlane && (col0 + xoff >= 0) && (col0 + xoff < L.M1);
-    int vsz[K], vcol[K];
-#pragma unroll
-    for (int q = 0; q < K; ++q) { vsz[q] = valid[q] ? 16 : 0; vcol[q] = valid[q] ? col0 + q : 0; }
-    const int xsz = xvalid ? 16 : 0, xcol = xvalid ? col0 + xoff : 0;
-    const unsigned x_ring = ch.in_ring - (unsigned)lane * 16u + (2 * K * 32 + (lane >> 4)) * 16;   // extra-column slot
+    const int wa = c0 - HALO, wb = wa - 1;              // first column of the A / B part of a record
+    const int ca0 = max(0, wa), ca1 = min(pitch, wa + Cfg::COLS);
+    const int cb0 = max(0, wb), cb1 = min(pitch, wb + Cfg::COLS + 2);
+    const unsigned nA = (unsigned)(ca1 - ca0) * 16u, nB = (unsigned)(cb1 - cb0) * 16u;
+    const unsigned dA = (unsigned)(ca0 - wa) * 16u, dB = (unsigned)(Cfg::COLS + cb0 - wb) * 16u;   // offsets in a record
     unsigned tpre = ch.t_in;                            // record counter of the prefetch
     int rpre = rho_start;                               // its iteration
+    if (FIRST && (nA != Cfg::COLS * 16 || nB != (Cfg::COLS + 2) * 16)) {   // first / last strip of a row
+        for (int e = lane; e < DIN * REC; e += 32) sts_d2_volatile(ch.in_ring + (unsigned)e * 16u, zero);
+        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");   // generic writes before the bulk copies' writes
+    }
+    __syncwarp();
     auto prefetch = [&]() {
         if (FIRST) {
-            if (rpre <= rho_end) {
-                const unsigned so = (tpre & (DIN - 1)) * RB;
+            __syncwarp();                               // every lane is done with the record that lived in this slot
+            if (lane == 0 && rpre <= rho_end) {
+                const unsigned slot = tpre & (DIN - 1);
+                const unsigned dst = ch.in_ring + slot * RB, bar = ch.in_bars + slot * 8;
                 const bool okh = (unsigned)(rpre + 2) <= (unsigned)rh_max, okf = (unsigned)(rpre + 1) <= (unsigned)rf_max;
-                const double2* ph = Hin + (okh ? (rpre + 2) * pitch : 0);
-                const double2* pf = Hin + Y + (okf ? (rpre + 1) * pitch : 0);
-#pragma unroll
-                for (int q = 0; q < K; ++q) {
-                    cp_async16_ca_sz(ch.in_ring + so + q * 512, ph + vcol[q], okh ? vsz[q] : 0);
-                    cp_async16_ca_sz(ch.in_ring + so + (K + q) * 512, pf + vcol[q], okf ? vsz[q] : 0);
-                }
-                cp_async16_ca_sz_if(x_ring + so, pf + xcol, okf ? xsz : 0, xlane);
+                mbar_arrive_expect_tx(bar, (okh ? nA : 0u) + (okf ? nB : 0u));
+                if (okh) bulk_g2s(dst + dA, Hin + ((rpre + 2) * pitch + ca0), nA, bar);
+                if (okf) bulk_g2s(dst + dB, Hin + (Y + (rpre + 1) * pitch + cb0), nB, bar);
             }
-            cp_async_commit();
             ++tpre; ++rpre;
         }
     };
@@ -227,6 +245,8 @@ __device__ __forceinline__ void regsweep_segment(const Layout& L, const int sys,
 #pragma unroll
         for (int v = 0; v < DPRE; ++v) prefetch();
     }
+    const unsigned a_lane = ch.in_ring + (unsigned)lane * (K * 16);                      // this lane's A columns
+    const unsigned x_lane = ch.in_ring + (Cfg::COLS + (lane == 31 ? Cfg::COLS + 1 : 0)) * 16;   // lanes 0 / 31: extra F^0 column
 
     // ---- role S-1: results -> HBM ----------------------------------------------------------------------
     double2* __restrict__ Hout = state_ptr(L, nxt, 0, sys) + col0;
@@ -243,6 +263,7 @@ __device__ __forceinline__ void regsweep_segment(const Layout& L, const int sys,
     int rho = rho_start;
     double nd0 = (double)(rho - j0);                    // row finished by stage j0, as double
     int o_out = (rho - j0) * pitch;                     // its element offset (stores of role S-1)
+    const double* cnp = cn0 + (rho - j0 + 2);           // c_n of the row started by stage j0 (stage j0 + 1: two rows back)
 
     // One stage: src = row n + 1 of the stencil grid, ownp = own pairs of row n + 2; finishes row n, starts row n + 2.
     auto stage = [&](auto edge_tag, auto par_tag, auto jl_tag, const double2* src, const double2* ownp, const int n,
@@ -309,7 +330,7 @@ __device__ __forceinline__ void regsweep_segment(const Layout& L, const int sys,
                 for (int q = 0; q < K; ++q) P[jl][0][q] = P[jl][1][q];
             }
             if (strt) {
-                const double cj = __ldg(cn0 + (n + 2));
+                const double cj = __ldg(cnp - 2 * jl);                // c_{n+2}
                 const double nd2 = nd + 2.0;
 #pragma unroll
                 for (int q = 0; q < K; ++q) {
@@ -336,23 +357,31 @@ __device__ __forceinline__ void regsweep_segment(const Layout& L, const int sys,
         // ---- take record rho ----
         double2 A[K], B[K], Fx = zero;
         if (!EDGE || rho <= rho_end) {
-            unsigned src;
             if (FIRST) {
                 prefetch();
-                cp_async_wait<DPRE>();                  // this lane's copies of record rho have landed
-                src = ch.in_ring + (ch.t_in & (DIN - 1)) * RB;
+                const unsigned slot = ch.t_in & (DIN - 1);
+                while (!mbar_try_wait(ch.in_bars + slot * 8, (ch.t_in / DIN) & 1u)) {}   // record rho has landed
+                const unsigned src = a_lane + slot * RB;
+                bool okh = true, okf = true;
+                if (EDGE) { okh = (unsigned)(rho + 2) <= (unsigned)rh_max; okf = (unsigned)(rho + 1) <= (unsigned)rf_max; }
+#pragma unroll
+                for (int q = 0; q < K; ++q) {
+                    A[q] = okh ? lds_d2_volatile(src + q * 16) : zero;
+                    B[q] = okf ? lds_d2_volatile(src + (Cfg::COLS + 1 + q) * 16) : zero;
+                }
+                Fx = okf ? lds_d2_volatile(x_lane + slot * RB) : zero;
+                ++ch.t_in;
             } else {
                 while ((int)(ch.prod_seen - ch.t_in) <= 0) ch.prod_seen = lds_u32_acquire(ch.in_flags);
-                src = ch.in_ring + (ch.t_in & (DF - 1)) * RB;
-            }
+                const unsigned src = ch.in_ring + (unsigned)lane * 16u + (ch.t_in & (DF - 1)) * RB;
 #pragma unroll
-            for (int q = 0; q < K; ++q) {
-                A[q] = lds_d2_volatile(src + q * 512);
-                B[q] = lds_d2_volatile(src + (K + q) * 512);
+                for (int q = 0; q < K; ++q) {
+                    A[q] = lds_d2_volatile(src + q * 512);
+                    B[q] = lds_d2_volatile(src + (K + q) * 512);
+                }
+                ++ch.t_in;
+                sts_u32_volatile(ch.in_flags + 128, ch.t_in);               // slot free again
             }
-            if (FIRST) Fx = lds_d2_volatile(x_ring + (ch.t_in & (DIN - 1)) * RB);
-            ++ch.t_in;
-            if (!FIRST) sts_u32_volatile(ch.in_flags + 128, ch.t_in);       // slot free again
         } else {
 #pragma unroll
             for (int q = 0; q < K; ++q) A[q] = B[q] = zero;
@@ -375,7 +404,7 @@ __device__ __forceinline__ void regsweep_segment(const Layout& L, const int sys,
 #pragma unroll
         for (int q = 0; q < K; ++q) { Zp[q] = Z0[q]; Bp[q] = B[q]; }
         ++rho; nd0 += 1.0;
-        o_out += pitch;
+        o_out += pitch; ++cnp;
     };
 
     using P0 = std::integral_constant<int, 0>;
@@ -432,19 +461,20 @@ __global__ void __launch_bounds__(RegCfg<S, K>::T, 1) regsweep_kernel(const __gr
     const unsigned ups = (unsigned)S * (unsigned)n_strips * (unsigned)rows;   // row-units per system, every role counts
     const long long upb = (long long)n_bands * rows;                          // band-rows per system
 
-    // shared memory: per team the input ring and S-1 FIFOs, then the counters, then per-warp reduction slots
     const unsigned smem0 = (unsigned)__cvta_generic_to_shared(rs_smem);
     const unsigned team_base = smem0 + (unsigned)team * (Cfg::TEAM_D2 * 16);
-    const unsigned flags0 = smem0 + (unsigned)STRIPS * (Cfg::TEAM_D2 * 16) + (unsigned)team * (Cfg::TEAM_FLAGS * 4);
-    double* accs = (double*)((char*)rs_smem + (size_t)STRIPS * (Cfg::TEAM_D2 * 16 + Cfg::TEAM_FLAGS * 4)) + warp * 64;
+    const unsigned flags0 = smem0 + (unsigned)Cfg::off_flags + (unsigned)team * (Cfg::TEAM_FLAGS * 4);
+    double* accs = (double*)((char*)rs_smem + Cfg::off_accs) + warp * 64;
     RegChan ch;
-    ch.in_ring = team_base + (role == 0 ? 0u : (unsigned)(Cfg::DIN + (role - 1) * Cfg::DF) * (Cfg::REC * 16)) + (unsigned)lane * 16u;
+    ch.in_ring = team_base + (role == 0 ? 0u : (unsigned)(Cfg::DIN + (role - 1) * Cfg::DF) * (Cfg::REC * 16));
     ch.out_ring = team_base + (unsigned)(Cfg::DIN + role * Cfg::DF) * (Cfg::REC * 16) + (unsigned)lane * 16u;
+    ch.in_bars = smem0 + (unsigned)Cfg::off_bars + (unsigned)team * (Cfg::DIN * 8);
     ch.in_flags = flags0 + (unsigned)(role > 0 ? role - 1 : 0) * 256u + (unsigned)lane * 4u;
     ch.out_flags = flags0 + (unsigned)(role < S - 1 ? role : 0) * 256u + (unsigned)lane * 4u;
     ch.t_in = 0; ch.t_out = 0; ch.prod_seen = 0; ch.cons_seen = 0;
-    for (int e = i; e < STRIPS * Cfg::TEAM_FLAGS; e += T)
-        sts_u32_volatile(smem0 + (unsigned)STRIPS * (Cfg::TEAM_D2 * 16) + (unsigned)e * 4u, 0u);
+    for (int e = i; e < STRIPS * Cfg::TEAM_FLAGS; e += T) sts_u32_volatile(smem0 + (unsigned)Cfg::off_flags + (unsigned)e * 4u, 0u);
+    if (i < STRIPS * Cfg::DIN) mbar_init(smem0 + (unsigned)Cfg::off_bars + (unsigned)i * 8u, 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
 
     // ---- active systems and this CTA's range of band-rows --------------------------------------------
     long long n_active = L.n_batch;
@@ -491,7 +521,7 @@ __global__ void __launch_bounds__(RegCfg<S, K>::T, 1) regsweep_kernel(const __gr
         start = min((long long)blockIdx.x * U, units);
         end = min(start + U, units);
     }
-    __syncthreads();   // counters zeroed, list visible
+    __syncthreads();   // counters zeroed, mbarriers initialised, list visible
 
     // ---- every warp walks the CTA's range segment by segment: its team's strip of the band, its role's step ----
     long long pos = start;

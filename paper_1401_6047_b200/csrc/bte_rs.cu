@@ -1,6 +1,7 @@
 // bte_rs.cu -- host side of the real-space-phi_x variant (include/bte.h, bte_rs_* entry points).
 // Product code: must not include, link or call anything under oracle/.
 #include "../../include/bte.h"
+#include "bte_internal.h"
 #include "bte_realspace.cuh"
 
 #include <cmath>
@@ -9,7 +10,6 @@
 
 using namespace bte;
 
-extern "C" void bte_internal_set_error(const char* text);   // bte.cu: thread-local text behind bte_last_error()
 
 namespace {
 

@@ -37,6 +37,16 @@ def test_every_declared_symbol_is_exported(lib):
     assert sorted(binding.EXPORTS) == names, "binding.EXPORTS must list exactly the header's functions"
 
 
+def test_exported_symbols_are_exactly_the_header(lib):
+    """-fvisibility=hidden + BTE_API: the dynamic symbol table of the .so holds the header's functions and nothing else."""
+    import subprocess
+    from paper_1401_6047_b200 import binding
+    out = subprocess.run(["nm", "-D", "--defined-only", binding.LIB_PATH], capture_output=True, text=True, check=True).stdout
+    exported = sorted(ln.split()[-1] for ln in out.splitlines() if len(ln.split()) >= 3 and ln.split()[-2] in ("T", "W", "B", "D"))
+    exported = [n for n in exported if not n.startswith("_")]          # toolchain symbols (_init, _fini, ...)
+    assert exported == declared_functions(), set(exported) ^ set(declared_functions())
+
+
 def test_struct_layouts_match_header():
     from paper_1401_6047_b200 import binding
     assert C.sizeof(binding.bte_grid) == 24            # 4 x int32 + double
@@ -89,6 +99,9 @@ def test_create_validates_before_touching_cuda(lib):
     rc, out = _create(lib, binding.make_grid(4, 41, 1, 0.5), binding.make_params(bad.params))
     assert rc == -2 and not out.value and b"unstable" in lib.bte_last_error()               # BTE_EUNSTABLE
     assert lib.bte_step(None, 1) == -1 and lib.bte_destroy(None) == 0
+    v = C.c_int64()
+    assert lib.bte_get_option(None, b"variant", C.byref(v)) == -1
+    assert lib.bte_get_state_batch(None, 0, None, None) == -1 and lib.bte_set_state_batch(None, 0, None, None) == -1
 
 
 def test_product_path_fails_loudly_without_a_gpu():

@@ -22,24 +22,43 @@ def run_bench(*extra):
 def test_default_workload_line():
     d = run_bench("--steps", "60", "--warmup", "3")
     for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
-              "vs_baseline", "dtype", "data", "config", "roofline", "cpu_baseline", "e2e", "gpu_launches", "clocks"):
+              "vs_baseline", "dtype", "data", "config", "roofline", "cpu_baseline", "e2e", "gpu_launches", "clocks",
+              "configs"):
         assert k in d, k
     assert d["config"]["workload"] == "config4_bandwidth_stress" and d["dtype"] == "f64" and d["n_gpus"] == 1
-    assert d["steps"] == 60 and d["gpu_launches"] == 20                       # 3 time steps per launch
+    assert set(d["config"]) == {"workload", "n_harm", "n_phiy", "n_batch", "dt", "name", "n_steps", "note"}   # = reference arm's
     r = d["roofline"]
+    S = round(r["steps_per_launch"])
+    assert d["steps"] == 60 and d["gpu_launches"] == 60 // S and S in (2, 3, 4)     # S time steps per launch
     assert r["bound"] == "hbm" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
-    assert r["kernel"] == "sweep_kernel" and r["traffic"] and 0.3 < r["frac"] < 1.1
+    assert r["kernel"] in ("sweep_kernel", "regsweep_kernel") and 0.3 < r["frac"] < 1.1
     assert r["one_step_per_pass"]["launches"] == r["one_step_per_pass"]["steps"]
     assert 0.5 < r["one_step_per_pass"]["frac"] < 1.1                         # the HBM-bound form of the kernel
     e = d["e2e"]
     assert e["unit"] == d["unit"] and 0 < e["value"] < d["value"] and e["h2d_bytes_per_step"] > 0 < e["d2h_bytes_per_step"]
     cb = d["cpu_baseline"]
     assert cb["kind"] == "oracle" and cb["cores"] >= 1 and 0 < cb["value"] < d["value"]
-    assert d["clocks"] is None or set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+    # the clock record must exist on the GPU box: median SM clock under load, max clock, throttle reasons
+    c = d["clocks"]
+    assert c is not None and c["samples"] >= 5 and c["sm_mhz"] > 0 and c["sm_max_mhz"] >= c["sm_mhz"] and isinstance(c["reasons"], list)
     assert abs(d["check"]["norm"] - 1.0) < 1e-10
+    # every other BASELINE config is timed in the same run, with its own norm check
+    assert set(d["configs"]) == {"config3_batched_sweep", "config2_paper_scale", "config1_crossed_ac", "config0_dc_B0"}
+    for name, c in d["configs"].items():
+        assert c["value"] > 0 and c["gpu_launches"] >= 1 and abs(c["check"]["norm"] - 1.0) < 1e-9, name
+        assert c["roofline"]["bound"] in ("hbm", "alu") and 0 < c["roofline"]["frac"] < 1.2, name
+    assert d["configs"]["config3_batched_sweep"]["roofline"]["bound"] == "hbm"
+    assert d["configs"]["config0_dc_B0"]["roofline"]["kernel"] == "resident_kernel"
 
 
 def test_resident_workload_line():
-    d = run_bench("--workload", "1", "--steps", "400", "--warmup", "3", "--no-cpu-baseline")
+    d = run_bench("--workload", "1", "--steps", "400", "--warmup", "3", "--no-cpu-baseline", "--no-other-configs")
     assert d["gpu_launches"] == 1 and d["roofline"]["kernel"] == "resident_kernel" and d["roofline"]["bound"] == "alu"
     assert d["e2e"]["value"] > 0 and abs(d["check"]["norm"] - 1.0) < 1e-10
+
+
+def test_cross_check_variant_is_labelled_by_what_ran():
+    d = run_bench("--steps", "6", "--warmup", "3", "--variant", "1", "--no-cpu-baseline", "--no-other-configs")
+    r = d["roofline"]
+    assert r["kernel"].startswith("half_update_kernel") and d["gpu_launches"] == 18     # 3 launches per step
+    assert abs(r["algorithmic_bytes_per_launch"] - 96.0 * 513 * 32001) < 1.0          # 96 B per point and step
