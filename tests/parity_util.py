@@ -69,6 +69,17 @@ def tucker_averages(mu, E_dc, E_w, w, nmax=60):
     return v_mean, v_cos, 2.0 / r * v_cos
 
 
+def tucker_sin_average(mu, E_dc, E_w, w, nmax=60):
+    """The quadrature partner of eq. (43) at B = 0 (same derivation: v(t) = (I1/I0) Im sum_{n,m} J_n J_m
+    e^{i (n-m) w t} / (1 - i (E_dc + m w)); <e^{i(n-m)wt} sin wt> = -+ 1/(2i) for n - m = +-1):
+    <v sin wt> = (I1/2I0) sum_n J_n(b) [J_{n+1}(b) - J_{n-1}(b)] / (1 + (E_dc + n w)^2),  b = E_w / w."""
+    nn = np.arange(-nmax, nmax + 1)
+    beta = E_w / w
+    J, Jp, Jm = special.jv(nn, beta), special.jv(nn + 1, beta), special.jv(nn - 1, beta)
+    r = float(special.ive(1, mu) / special.ive(0, mu))
+    return 0.5 * r * float(np.sum(J * (Jp - Jm) / (1 + (E_dc + nn * w) ** 2)))
+
+
 def absorption(obs, mu):
     """Eq. (17): A = (2 I0(mu)/I1(mu)) <v_dr cos wt>, from the raw sums the library returns (C9)."""
     return 2.0 * float(special.ive(0, mu) / special.ive(1, mu)) * obs.sum_vcos_dt / obs.window

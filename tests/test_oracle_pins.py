@@ -273,6 +273,12 @@ def test_P9_tucker_time_averages():
     assert abs(o.window - n_avg * dt) < 1e-9
     assert abs(o.sum_v_dt / o.window - v_mean) < 2e-4 * abs(v_mean)
     assert abs(o.sum_vcos_dt / o.window - v_cos) < 2e-3 * abs(v_cos) + 1e-6
+    # the third accumulator, sum v sin(wt) dt: the quadrature partner of eq. (43) -- in the derivation of (42)-(43),
+    # v(t) = (I1/I0) Im sum_{n,m} J_n J_m e^{i(n-m)wt} / (1 - i(E_dc + m w)), the sin wt average picks n - m = +-1 with
+    # weights -+1/(2i), which leaves (I1/2I0) sum_n J_n [J_{n+1} - J_{n-1}] / (1 + (E_dc + n w)^2)
+    v_sin = 0.5 * r * np.sum(J * (Jp - Jm) / (1 + (E_dc + nn * w) ** 2))
+    assert abs(v_sin) > 3 * abs(v_cos) > 0                      # cos / sin swapped or a wrong sign cannot pass
+    assert abs(o.sum_vsin_dt / o.window - v_sin) < 2e-3 * abs(v_sin) + 1e-6
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -507,10 +513,35 @@ def test_pendulum_ac_B0_is_tucker_at_T0():
     from oracle import pendulum_averages
     from parity_util import tucker_averages
     E_dc, E_w, w = 2.0, 0.5, 1.5
+    from parity_util import tucker_sin_average
     v, vc, vs = pendulum_averages(E_dc, E_w, w, 0.0, 64, 0.004, 10000)
     r = float(special.ive(1, 1e6) / special.ive(0, 1e6))       # -> 1
     v_ref, vc_ref, _ = tucker_averages(1e6, E_dc, E_w, w)
+    vs_ref = tucker_sin_average(1e6, E_dc, E_w, w)
     assert abs(v - v_ref / r) < 1e-9 and abs(vc - vc_ref / r) < 1e-9
+    assert abs(vs_ref) > 3 * abs(vc_ref) and abs(vs - vs_ref / r) < 1e-9        # third output: <v_dr sin wt>
+
+
+def test_P11_low_temperature_oracle_approaches_the_pendulum_model():
+    """P11 (Fig. 4b parameters B = 4, E_dc = 6, E_omega = 0.1, alpha = 0.9496, mu = 116): the
+    oracle's time averages against the T = 0 pendulum model (itself pinned by the closed forms above), on a lattice
+    small enough for the CPU suite.  "Very close, but not quite, due to the finite temperature" (L225): <v_dr> within
+    2 %, the absorption within 15 % of the pendulum value."""
+    from oracle import pendulum_averages
+    from parity_util import absorption
+    mu, E_dc, E_w, B, alpha, om, dt = 116.0, 6.0, 0.1, 4.0, 0.9496, 5.0, 0.004
+    n_relax = int(round(10.0 / dt))
+    n_avg = int(round(4 * 2 * math.pi / (om * dt)))
+    s, _ = make(64, 501, dt, E_dc=E_dc, E_omega=E_w, omega=om, B=B, mu=mu, alpha=alpha, phiy_min=-5.0, phiy_max=5.0,
+                avg_start_step=n_relax)
+    s.init_equilibrium()
+    s.step(n_relax + n_avg)
+    o = s.observables()
+    v_p, vc_p, vs_p = pendulum_averages(E_dc, E_w, om, B, 64, 0.004, 10000)
+    assert abs(o.norm - 1.0) < 1e-6
+    assert abs(o.sum_v_dt / o.window - v_p) < 0.02 * abs(v_p)
+    assert abs(absorption(o, mu) - 2.0 * vc_p) < 0.15 * max(abs(2.0 * vc_p), 0.02)
+    assert abs(o.sum_vsin_dt / o.window - vs_p) < 0.15 * max(abs(vs_p), 0.01)
 
 
 def test_pendulum_energy_invariant_and_phase_count():

@@ -70,3 +70,22 @@ def test_second_order_convergence_to_the_harmonic_form():
         err.append(abs(s.v_dr() - v_ref))
     assert 3.3 < err[0] / err[1] < 4.7 and 3.3 < err[1] / err[2] < 4.7, err
     assert err[2] < 2e-3 * abs(v_ref)
+
+
+def test_running_sums_match_the_harmonic_form():
+    """sum v dt, sum v cos(wt) dt, sum v sin(wt) dt of the real-space oracle against the harmonic-form oracle (whose
+    three sums are pinned by the Tucker closed forms, P9): same problem, ac field, K = 64 phi_x points (dx^2 error)."""
+    kw = dict(N=24, M1=41, dt=0.005, E_dc=2.0, E_omega=0.5, omega=1.5, B=1.0, mu=2.0, phiy_max=6.0, avg_start=40)
+    p = params(**kw)
+    ref = OracleSim(24, 41, 0.005, p)
+    ref.init_equilibrium()
+    ref.step(240)
+    o = ref.observables()
+    s = RealSpaceSim(64, 41, 0.005, p)
+    s.init_equilibrium()
+    s.step(240)
+    assert abs(s.window - o.window) < 1e-12 and o.window > 0.9
+    assert min(abs(o.sum_vcos_dt), abs(o.sum_vsin_dt)) > 0.02 * abs(o.sum_v_dt)   # all three sums are significant here
+    assert abs(o.sum_vcos_dt - o.sum_vsin_dt) > 0.02 * abs(o.sum_v_dt)            # ... and distinguishable
+    for got, want in ((s.sum_v, o.sum_v_dt), (s.sum_c, o.sum_vcos_dt), (s.sum_s, o.sum_vsin_dt)):
+        assert abs(got - want) < 3e-3 * abs(o.sum_v_dt), (got, want)
