@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libbte_b200.so")
 SOURCES = [os.path.join(CSRC, "bte.cu"), os.path.join(CSRC, "bte_rs.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("bte_device.cuh", "bte_kernels.cuh", "bte_internal.h", "bte_sweep.cuh", "bte_regsweep.cuh", "bte_resident.cuh", "bte_pendulum.cuh", "bte_lowprec.cuh", "bte_realspace.cuh")] + \
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("bte_device.cuh", "bte_kernels.cuh", "bte_internal.h", "bte_sweep.cuh", "bte_warpsweep.cuh", "bte_resident.cuh", "bte_pendulum.cuh", "bte_lowprec.cuh", "bte_realspace.cuh")] + \
     [os.path.join(os.path.dirname(HERE), "include", "bte.h")]
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

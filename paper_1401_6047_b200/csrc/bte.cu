@@ -3,7 +3,7 @@
 #include "../../include/bte.h"
 #include "bte_internal.h"
 #include "bte_sweep.cuh"
-#include "bte_regsweep.cuh"
+#include "bte_warpsweep.cuh"
 #include "bte_resident.cuh"
 #include "bte_pendulum.cuh"
 #include "bte_lowprec.cuh"
@@ -234,21 +234,21 @@ SweepFn sweep_fn(int S, bool budgets, int wide) {
     }
 }
 constexpr int RING_MAX_STEPS = 3;   // the shared-memory-ring kernel is instantiated for S = 1 .. 3
-static_assert(SWEEP_MAX_STEPS == 4, "instantiate regsweep_kernel for every S from 2 up to SWEEP_MAX_STEPS");
+constexpr int WS_MAX_STEPS = 3;     // the register-resident kernel is instantiated for S = 2, 3
+static_assert(WS_MAX_STEPS <= SWEEP_MAX_STEPS, "partial sums are laid out for SWEEP_MAX_STEPS steps per pass");
 
-// register-pipelined kernel (bte_regsweep.cuh): S = 2 .. SWEEP_MAX_STEPS steps per pass, K = 2 columns per lane
+// register-resident warp kernel (bte_warpsweep.cuh): S = 2, 3 steps per pass, K = 2 columns per lane
 constexpr int RS_K = 2;
 template <int S>
 SweepFn regsweep_fn_s(bool budgets) {
-    using Cfg = RegCfg<S, RS_K>;
-    return {budgets ? (void*)regsweep_kernel<S, RS_K, true> : (void*)regsweep_kernel<S, RS_K, false>,
-            Cfg::smem_bytes, Cfg::W, Cfg::T, Cfg::STRIPS};
+    using Cfg = WarpCfg<S, RS_K>;
+    return {budgets ? (void*)warpsweep_kernel<S, RS_K, true> : (void*)warpsweep_kernel<S, RS_K, false>,
+            Cfg::smem_bytes, Cfg::W, Cfg::T, Cfg::WARPS};
 }
 SweepFn regsweep_fn(int S, bool budgets) {
     switch (S) {
         case 2: return regsweep_fn_s<2>(budgets);
-        case 3: return regsweep_fn_s<3>(budgets);
-        default: return regsweep_fn_s<4>(budgets);
+        default: return regsweep_fn_s<3>(budgets);
     }
 }
 
@@ -270,27 +270,27 @@ int plan_sweep(bte_ctx* c) {
     c->sm_count = sms;
     const long long rows_alloc = c->grid.n_harm + 1 + 2 * GHOST;
     // register-pipelined kernel: one CTA (teams of S warps) per SM; a CTA range is counted in band-rows
-    for (int S = 2; S <= SWEEP_MAX_STEPS; ++S) {
+    for (int S = 2; S <= WS_MAX_STEPS; ++S) {
         const SweepFn f = regsweep_fn(S, c->has_budgets);
         int occ = 0;
         cudaError_t e = cudaFuncSetAttribute(f.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f.smem);
         if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f.fn, f.T, f.smem);
         if (e != cudaSuccess)
-            return fail(BTE_ECUDA, "regsweep_kernel<S=%d> setup failed: %s (is this an sm_100a device?)", S,
+            return fail(BTE_ECUDA, "warpsweep_kernel<S=%d> setup failed: %s (is this an sm_100a device?)", S,
                         cudaGetErrorString(e));
         if (occ < 1) continue;
         const long long strips = (c->grid.n_phiy + f.W - 1) / f.W;
         const long long bands = (strips + f.strips_per_band - 1) / f.strips_per_band;
         const long long units = bands * (c->grid.n_harm + 1) * (long long)c->grid.n_batch;
         if (2LL * c->grid.n_batch * rows_alloc * c->off.pitch >= (1LL << 31)) continue;   // 32-bit element offsets
-        if (S * strips * (c->grid.n_harm + 1) >= (1LL << 31) || units >= (1LL << 31)) continue;
+        if (strips * (c->grid.n_harm + 1) >= (1LL << 31) || units >= (1LL << 31)) continue;
         long long g = (long long)sms * occ;
         // a segment costs about NS + HALO extra row iterations: a CTA should own a few times that many rows
         const long long min_rows = c->sweep_ctas > 0 ? 1 : 8 * S;
         if (c->sweep_ctas > 0) g = c->sweep_ctas;
         if (g > (units + min_rows - 1) / min_rows) g = (units + min_rows - 1) / min_rows;
         if (g < 1) g = 1;
-        if (c->has_budgets && (long long)c->grid.n_batch / g + 2 > RegCfg<2, RS_K>::MAX_SPAN) continue;
+        if (c->has_budgets && (long long)c->grid.n_batch / g + 2 > WarpCfg<2, RS_K>::MAX_SPAN) continue;
         c->rs_grid[S] = (int)g;
     }
     for (int S = 1; S <= RING_MAX_STEPS; ++S) {

@@ -1,0 +1,507 @@
+// bte_warpsweep.cuh -- streaming kernel of libbte_b200 (sm_100a): S leap-frog steps per pass over the lattice,
+// every warp an independent register-resident pipeline of all 2 S half-updates.
+//
+// One launch = S consecutive leap-frog steps (eq. 40-41) of every active system = NS = 2 S applications of T
+// (eq. 38), alternating whole / fractional grid, in one pass over the lattice: 64/S bytes of HBM traffic per
+// lattice point per time step (ping-pong buffers), as in bte_sweep.cuh.  What differs is where the intermediate
+// time levels live.  bte_sweep.cuh passes every stage row between the threads of a CTA through shared-memory rings
+// behind one CTA-wide barrier per row (72 B of shared-memory traffic per half-update: that pipe and the barrier are
+// its bound, profiles/r01e).  Here nothing but the HBM input ever touches shared memory:
+//
+// * a strip of 32 K adjacent phi_y columns belongs to ONE warp; lane l holds the K adjacent columns K l .. K l + K - 1
+//   of every time level; the warp marches over n;
+// * iteration rho: the warp takes one record from its input ring,
+//       A = X^{-1}[rho + 2] (row of H^0: own pairs of stage 0),   B = X^0[rho + 1] (row of F^0: stencil row of stage 0)
+//   and runs the NS stages one after the other, all in registers: stage j takes the phi_y-difference D of row
+//   rho - j + 1 of X^j (its own K columns; the two outer neighbours by warp shuffle), which FINISHES row rho - j of
+//   X^{j+1} (started two iterations ago) and, with the own pairs X^{j-1}[rho - j + 2] that stage j - 2 has formed in
+//   this very iteration, STARTS row rho - j + 2 (cn_complete / cn_partial, bte_device.cuh).  The only state carried
+//   between iterations is the partial right-hand side (Pg, Ph) of the two rows in flight per stage and column;
+// * no barrier, no flag, no fence anywhere in the march: warps never exchange data.  The first / last HALO = NS - 1
+//   columns of a strip are recomputed halos (W = 32 K - 2 HALO owned columns); segments that cut a column at an
+//   arbitrary row recompute HALO halo rows on each side (trapezoid in n as in m);
+// * HBM -> shared memory: lane 0 issues two 1-D bulk copies per record (TMA engine, SASS UBLKCP) DPRE records ahead
+//   into a per-warp ring, completion on the slot's mbarrier; zero rows / columns outside the lattice are never read
+//   (boundary conditions (22)-(23)).  Results go to HBM straight from registers (128-bit stores);
+// * mu^t_{n,m} = n beta^t_m dt/2 (eq. 28-29) is formed as fma(n, B phi_m dt/2, n E(t) dt/2): the column part is two
+//   registers per column, the field part one number per row and half-step time (E(t_v) dt/2 sits in shared memory,
+//   read as a broadcast), so that no per-column table of the NS + 2 half-step times is needed -- registers are for
+//   the NS x 2 x K partial right-hand sides.  mu of row n at time t_v is the implicit mu' of stage v - 2 and the
+//   explicit mu of stage v in the same iteration: formed once.
+//
+// Work decomposition: bands of WARPS adjacent strips; band-rows (system, band, n) are numbered consecutively and
+// dealt out in equal contiguous ranges to one CTA per SM; warp g of the CTA takes strip g of the band, so the warps
+// of a CTA touch adjacent 1 KB runs of every row (DRAM page locality).
+// Per-step reductions (eq. 12, 17, 20): the even stages see rows 0 and 1 of the new whole grids -> per-strip partial
+// sums -> fixed-order fold by the warp that completes a system (fold_sweep, bte_sweep.cuh).
+#pragma once
+#include <type_traits>
+
+#include "bte_sweep.cuh"
+
+namespace bte {
+
+template <int S, int K>
+struct WarpCfg {
+    static constexpr int NS = 2 * S;            // half-updates (stages) per pass
+    static constexpr int NV = NS + 2;           // half-step times of a pass
+    static constexpr int HALO = NS - 1;         // halo columns on each side of a strip, halo rows of a segment
+    static constexpr int COLS = 32 * K;         // columns a warp computes
+    static constexpr int W = COLS - 2 * HALO;   // owned columns per strip
+    static constexpr int WARPS = 8;             // warps per CTA = strips per band
+    static constexpr int T = 32 * WARPS;
+    static constexpr int DIN = 8;               // slots of the HBM input ring
+    static constexpr int DPRE = 6;              // rows prefetched ahead (the slot of record t + DPRE was read 2 iterations ago)
+    static constexpr int REC = 2 * COLS + 2;    // double2 per record: A = COLS columns, B = COLS + 2 columns, natural order
+    static constexpr int MAX_SPAN = 64;         // distinct systems one CTA range may touch
+    // shared memory of one warp: input ring | E(t_v) dt/2 at the NV half-step times | mbarriers | reduction slots [S][2][32]
+    static constexpr size_t off_tab = (size_t)DIN * REC * 16;
+    static constexpr size_t off_bars = off_tab + (size_t)NV * 8;
+    static constexpr size_t off_accs = off_bars + (size_t)DIN * 8;
+    static constexpr size_t warp_bytes = off_accs + (size_t)S * 2 * 32 * 8;
+    static constexpr size_t smem_bytes = (size_t)WARPS * warp_bytes;
+    static_assert(W >= 8, "strip too narrow");
+    static_assert((DIN & (DIN - 1)) == 0 && DPRE + 2 <= DIN, "ring sizes");
+    static_assert(warp_bytes % 16 == 0 && off_tab % 16 == 0, "alignment");
+};
+
+struct WarpShared {
+    int scan[16];
+    int list[64];
+    unsigned int flag;
+};
+
+__device__ __forceinline__ double2 shfl_up_d2(double2 v) {
+    double2 r;
+    r.x = __shfl_up_sync(0xffffffffu, v.x, 1);
+    r.y = __shfl_up_sync(0xffffffffu, v.y, 1);
+    return r;
+}
+__device__ __forceinline__ double2 shfl_down_d2(double2 v) {
+    double2 r;
+    r.x = __shfl_down_sync(0xffffffffu, v.x, 1);
+    r.y = __shfl_down_sync(0xffffffffu, v.y, 1);
+    return r;
+}
+__device__ __forceinline__ double2 lds_d2_volatile(unsigned addr) {
+    double2 v;
+    asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];\n" : "=d"(v.x), "=d"(v.y) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_d2_volatile(unsigned addr, double2 v) {
+    asm volatile("st.volatile.shared.v2.f64 [%0], {%1, %2};\n" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory");
+}
+// ---- 1-D bulk copies (TMA engine, SASS UBLKCP) with mbarrier completion: the HBM input ring ----
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(unsigned bar, unsigned parity) {
+    unsigned ok;
+    asm volatile(
+        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+// global -> shared, `bytes` a multiple of 16, both addresses 16-byte aligned; completion is signalled on `bar`
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+
+__device__ __forceinline__ bool elect_one() {
+    unsigned ok;
+    asm volatile("{\n .reg .pred p;\n elect.sync _|p, 0xffffffff;\n selp.u32 %0, 1, 0, p;\n}\n" : "=r"(ok));
+    return ok != 0;
+}
+// a value every lane holds anyway, re-broadcast from lane 0 so that the compiler KNOWS it is warp-uniform and keeps it
+// (and everything derived from it) in uniform registers: the bulk-copy operands must be uniform, and the vector
+// registers are needed for the partial right-hand sides
+__device__ __forceinline__ int uni(int v) { return __shfl_sync(0xffffffffu, v, 0); }
+__device__ __forceinline__ unsigned uni(unsigned v) { return __shfl_sync(0xffffffffu, v, 0); }
+
+// One segment of one warp: system sys, strip, rows r0 .. r0+Lr-1.
+//   ring, bars: shared addresses of this warp's input ring and mbarriers; tabp: its table of E(t_v) dt/2; accs: its
+//   reduction slots;
+//   t_in: records taken so far in this launch (slot and mbarrier phase of the next one).
+template <int S, int K>
+__device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys, const int strip, const int r0,
+                                                  const int Lr, const int n_strips, const unsigned ups,
+                                                  const unsigned ring, double* tabp, const unsigned bars,
+                                                  double* __restrict__ accs, unsigned& t_in) {
+    using Cfg = WarpCfg<S, K>;
+    constexpr int NS = Cfg::NS, NV = Cfg::NV, HALO = Cfg::HALO, W = Cfg::W, REC = Cfg::REC;
+    constexpr int DIN = Cfg::DIN, DPRE = Cfg::DPRE;
+    constexpr unsigned RB = REC * 16;                   // bytes per record
+    const int lane = threadIdx.x & 31;
+    const double2 zero = make_double2(0.0, 0.0);
+
+    const SysConst c = L.sc[sys];
+    const long long k = L.ss[sys].k;
+    const int cur = uni(L.ss[sys].buf), nxt = cur ^ 1;
+    const int N = L.N, pitch = L.pitch;
+    // the fractional grid of the same buffer sits Y elements further (Y < 2^30, checked by the host)
+    const int Y = L.n_batch * (N + 1 + 2 * GHOST) * pitch;
+    const int c0 = strip * W;
+    const int col0 = c0 - HALO + K * lane;              // this lane's first column
+    const double* __restrict__ cn0 = cn_ptr(L, sys);
+
+    bool own[K];
+    double gdt[K], kap[K], bph[K];                      // a^(0) prefactor g_m dt, kappa, B phi_m dt/2 of this lane's columns
+    {
+        // field at the NV half-step times of the pass (C14): lane v evaluates E(t_k + v dt/2) dt/2
+        if (lane < NV)
+            *(volatile double*)(&tabp[lane]) = __dmul_rn(field_E(c, ((double)k + 0.5 * (double)lane) * L.dt), L.hd);
+#pragma unroll
+        for (int q = 0; q < K; ++q) {
+            const int col = col0 + q, x = K * lane + q;
+            const bool valid = (col >= 0) && (col < L.M1);
+            own[q] = valid && (x >= HALO) && (x < HALO + W);
+            bph[q] = valid ? __dmul_rn(__dmul_rn(c.B, L.phi[(size_t)sys * pitch + col]), L.hd) : 0.0;
+            gdt[q] = valid ? __dmul_rn(L.gm[(size_t)sys * pitch + col], L.dt) : 0.0;
+            kap[q] = valid ? c.kappa_dt : 0.0;          // invalid columns: w = 0, src = 0, kappa = 0 => stay 0
+        }
+        __syncwarp();
+    }
+
+    // row ranges (trapezoid in n): stage j forms rows max(0, lo_base + j) .. min(N, hi_base - j)
+    const int lo_base = r0 - HALO, hi_base = r0 + Lr - 1 + HALO;
+    const int rho_start = max(0, lo_base) - 2;          // first / last iteration of the segment
+    const int rho_end = min(N, r0 + Lr - 1) + NS - 1;
+    // steady state: every stage finishes a row >= 1 and starts a row of its range, stores in range, full records
+    const int rho_s0 = NS - 1 + max(r0, 1);
+    const int rho_s1 = min(N, hi_base) - 2;
+
+    // ---- HBM -> input ring -------------------------------------------------------------------------------
+    // record rho = (A = H^0 row rho + 2, columns c0 - HALO .. + COLS - 1;  B = F^0 row rho + 1, one column more on
+    // each side), natural column order.  Columns outside [0, pitch) are not copied: those parts of the ring are
+    // zeroed once per segment (boundary condition (22)-(23) in m; the pad columns M+1 .. pitch-1 are zero in HBM).
+    // Rows outside the lattice / the segment's trapezoid are not copied either: the record reads as zero.
+    const double2* __restrict__ Hin = state_ptr(L, cur, 0, sys);   // row 0, column 0
+    const int rf_max = min(N, hi_base + 1), rh_max = min(N, hi_base);      // last F^0 / H^0 row needed
+    const int wa = c0 - HALO, wb = wa - 1;              // first column of the A / B part of a record
+    const int ca0 = max(0, wa), ca1 = min(pitch, wa + Cfg::COLS);
+    const int cb0 = max(0, wb), cb1 = min(pitch, wb + Cfg::COLS + 2);
+    const unsigned nA = (unsigned)(ca1 - ca0) * 16u, nB = (unsigned)(cb1 - cb0) * 16u;
+    const unsigned dA = (unsigned)(ca0 - wa) * 16u, dB = (unsigned)(Cfg::COLS + cb0 - wb) * 16u;   // offsets in a record
+    unsigned tpre = t_in;                               // record counter of the prefetch
+    int rpre = rho_start;                               // its iteration
+    if (nA != Cfg::COLS * 16 || nB != (Cfg::COLS + 2) * 16) {   // first / last strip of a row
+        for (int e = lane; e < DIN * REC; e += 32) sts_d2_volatile(ring + (unsigned)e * 16u, zero);
+        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");   // generic writes before the bulk copies' writes
+    }
+    __syncwarp();
+    // Rows outside the lattice / the trapezoid are clamped to the nearest row the segment reads anyway (the record is
+    // then read as zero, see `okh`, `okf` below): the prefetch is branch-free, two copies of fixed size per record.
+    const double2* gA = Hin + (min(max(rpre + 2, 0), rh_max) * pitch + ca0);
+    const double2* gF = Hin + (Y + min(max(rpre + 1, 0), rf_max) * pitch + cb0);
+    auto prefetch = [&]() {
+        // (the record that lived in this slot was read two iterations ago: those loads have long been consumed)
+        if (rpre <= rho_end && elect_one()) {
+            const unsigned slot = tpre & (DIN - 1);
+            const unsigned dst = ring + slot * RB, bar = bars + slot * 8;
+            mbar_arrive_expect_tx(bar, nA + nB);
+            bulk_g2s(dst + dA, gA, nA, bar);
+            bulk_g2s(dst + dB, gF, nB, bar);
+        }
+        if (rpre + 2 >= 0 && rpre + 2 < rh_max) gA += pitch;
+        if (rpre + 1 >= 0 && rpre + 1 < rf_max) gF += pitch;
+        ++tpre; ++rpre;
+    };
+#pragma unroll
+    for (int v = 0; v < DPRE; ++v) prefetch();
+    const unsigned a_lane = ring + (unsigned)lane * (K * 16);                             // this lane's A columns
+
+    // ---- results -> HBM ----------------------------------------------------------------------------------
+    double2* __restrict__ Hout = state_ptr(L, nxt, 0, sys) + col0;
+    double2* __restrict__ Fout = Hout + Y;
+
+    double2 P[NS][2][K];                                // partial right-hand sides in flight: [stage][slot][column]
+#pragma unroll
+    for (int j = 0; j < NS; ++j)
+#pragma unroll
+        for (int q = 0; q < K; ++q) P[j][0][q] = P[j][1][q] = zero;
+
+    int rho = rho_start;
+    double nd0 = (double)rho;                           // row finished by stage 0, as double
+    int o_out = (rho - (NS - 2)) * pitch;               // element offset of the row finished by stage NS - 2
+    const double* cnp = cn0 + (rho + 2);                // c_n of the row started by stage 0 (stage j: j rows back)
+
+    // edge_tag: std::true_type = fill / drain iteration (row predicates, special rows 0 and 1);
+    // par_tag: steady state only: which of the two slots of P is finished (and refilled) in this iteration
+    auto body = [&](auto edge_tag, auto par_tag) {
+        constexpr bool EDGE = decltype(edge_tag)::value;
+        constexpr int PAR = decltype(par_tag)::value;
+        // ---- take record rho ----
+        double2 Z[NS + 2][K];                           // Z[j + 2] = output of stage j; Z[0] = A, Z[1] = B
+        double2 FL, FR;                                 // F^0 columns left / right of this lane's K columns
+        {
+            prefetch();
+            const unsigned slot = t_in & (DIN - 1);
+            while (!mbar_try_wait(bars + slot * 8, (t_in / DIN) & 1u)) {}   // record rho has landed
+            const unsigned src = a_lane + slot * RB;
+            bool okh = true, okf = true;
+            if (EDGE) { okh = (unsigned)(rho + 2) <= (unsigned)rh_max; okf = (unsigned)(rho + 1) <= (unsigned)rf_max; }
+#pragma unroll
+            for (int q = 0; q < K; ++q) {
+                Z[0][q] = okh ? lds_d2_volatile(src + q * 16) : zero;
+                Z[1][q] = okf ? lds_d2_volatile(src + (Cfg::COLS + 1 + q) * 16) : zero;
+            }
+            FL = okf ? lds_d2_volatile(src + Cfg::COLS * 16) : zero;
+            FR = okf ? lds_d2_volatile(src + (Cfg::COLS + 1 + K) * 16) : zero;
+            ++t_in;
+        }
+        // mu[v][q] = n beta^{t_v}_m dt/2 of row n = rho - v + 2 (eq. 28-29): explicit mu of stage v, implicit mu' of stage v - 2
+        double mu[NV][K];
+        auto form_mu = [&](const int v) {
+            const double ndv = nd0 + (double)(2 - v);
+            const double ndE = __dmul_rn(ndv, *(volatile double*)(&tabp[v]));
+#pragma unroll
+            for (int q = 0; q < K; ++q) mu[v][q] = __fma_rn(ndv, bph[q], ndE);
+        };
+        form_mu(0);
+        form_mu(1);
+        form_mu(2);
+        double2 pq[NS][K];                              // (nu, mu') / (nu^2 + mu'^2) of stage j: formed one stage ahead
+#pragma unroll
+        for (int q = 0; q < K; ++q) pq[0][q] = cn_coef(mu[2][q], L.nu, L.nu2);
+#pragma unroll
+        for (int j = 0; j < NS; ++j) {
+            // src = Z[j + 1] = row n + 1 of the stencil grid X^j, ownp = Z[j] = own pairs of row n + 2;
+            // finishes row n = rho - j of X^{j+1}, starts row n + 2
+            const double2* src = Z[j + 1];
+            const double2* ownp = Z[j];
+            double2* Zo = Z[j + 2];
+            const int n = rho - j;
+            bool comp = true, strt = true;
+            if (EDGE) {
+                const int lo = max(0, lo_base + j), hi = min(N, hi_base - j);
+                comp = n >= lo && n <= hi;
+                strt = n + 2 >= lo && n + 2 <= hi;
+            }
+            // phi_y-difference of row n + 1 of the stencil grid: interior columns from registers, the two outer ones
+            // from the adjacent lanes (stage 0: from the ring)
+            double2 Lv, Rv;
+            if (j == 0) { Lv = FL; Rv = FR; }
+            else { Lv = shfl_up_d2(src[K - 1]); Rv = shfl_down_d2(src[0]); }
+            if (j + 1 < NS) {                                         // coefficients of the next stage: independent of
+                form_mu(j + 3);                                       // the data, they fill the latency of the shuffles
+#pragma unroll
+                for (int q = 0; q < K; ++q) pq[j + 1 < NS ? j + 1 : 0][q] = cn_coef(mu[j + 3][q], L.nu, L.nu2);
+            }
+            if (!EDGE || comp || strt) {
+                double2 D[K];
+#pragma unroll
+                for (int q = 0; q < K; ++q) {
+                    const double2 r = (q + 1 < K) ? src[q + 1 < K ? q + 1 : 0] : Rv;
+                    const double2 l = (q > 0) ? src[q > 0 ? q - 1 : 0] : Lv;
+                    D[q].x = __dsub_rn(r.x, l.x);
+                    D[q].y = __dsub_rn(r.y, l.y);
+                }
+                if (comp) {
+#pragma unroll
+                    for (int q = 0; q < K; ++q) {
+                        const double2 Pq = EDGE ? P[j][0][q] : P[j][PAR][q];
+                        Zo[q] = cn_apply(Pq, D[q], kap[q], pq[j][q]);
+                        if (EDGE && n == 0) Zo[q].y = 0.0;            // b_0 == 0 (eq. 23, C3)
+                    }
+                    const bool mine = !EDGE || (n >= r0 && n < r0 + Lr);
+                    if (j >= NS - 2 && mine) {                        // the two newest time levels go to HBM
+                        double2* out = (j == NS - 1) ? Fout + (o_out - pitch) : Hout + o_out;
+#pragma unroll
+                        for (int q = 0; q < K; ++q)
+                            if (own[q]) out[q] = Zo[q];
+                    }
+                    if (EDGE && (j & 1) == 0 && mine && n <= 1) {     // whole grid of step k + j/2 + 1: reductions
+                        double v = 0.0;
+#pragma unroll
+                        for (int q = 0; q < K; ++q)
+                            if (own[q]) v += (n == 0) ? Zo[q].x : Zo[q].y;
+                        accs[((j >> 1) * 2 + n) * 32 + lane] = v;
+                        if (j == NS - 2 && n == 1) {
+#pragma unroll
+                            for (int q = 0; q < K; ++q) {
+                                if (own[q] && col0 + q == 0) L.ss[sys].edge[0] = fabs(Zo[q].y);
+                                if (own[q] && col0 + q == L.M1 - 1) L.ss[sys].edge[1] = fabs(Zo[q].y);
+                            }
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int q = 0; q < K; ++q) Zo[q] = zero;         // outside the lattice / this segment's halo
+                }
+                if (EDGE) {
+#pragma unroll
+                    for (int q = 0; q < K; ++q) P[j][0][q] = P[j][1][q];
+                }
+                if (strt) {
+                    const double cj = __ldg(cnp - j);                 // c_{n+2}
+#pragma unroll
+                    for (int q = 0; q < K; ++q) {
+                        double2 lo = D[q];
+                        if (EDGE && n + 2 == 1) lo.x *= 2.0;          // chi(1) = 2, eq. (11)
+                        const double2 Pn = cn_partial(ownp[q], lo, mu[j][q], __dmul_rn(cj, gdt[q]), kap[q], L.xi);
+                        if (EDGE) P[j][1][q] = Pn; else P[j][PAR][q] = Pn;
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int q = 0; q < K; ++q) {
+                    Zo[q] = zero;
+                    P[j][0][q] = P[j][1][q];
+                }
+            }
+        }
+        ++rho; nd0 += 1.0;
+        o_out += pitch; ++cnp;
+    };
+
+    using P0 = std::integral_constant<int, 0>;
+    using P1 = std::integral_constant<int, 1>;
+    while (rho <= rho_end && rho < rho_s0) body(std::true_type{}, P0{});
+    while (rho + 1 <= rho_s1) {                         // two iterations per trip: the slots of P alternate
+        body(std::false_type{}, P0{});
+        body(std::false_type{}, P1{});
+    }
+    while (rho <= rho_end) body(std::true_type{}, P0{});
+
+    // per-strip partial sums of row 0 (a) and row 1 (b) of the S new whole grids -> eq. (12), (20)
+    const bool has0 = (r0 == 0), has1 = (r0 <= 1) && (r0 + Lr > 1);
+    if (has0 || has1) {
+        __syncwarp();
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            double* part = L.partial + (((size_t)s * L.n_batch + sys) * pitch + strip) * 2;
+            if (has0) {
+                const double v = warp_sum(accs[(s * 2 + 0) * 32 + lane]);
+                if (lane == 0) part[0] = v;
+            }
+            if (has1) {
+                const double v = warp_sum(accs[(s * 2 + 1) * 32 + lane]);
+                if (lane == 0) part[1] = v;
+            }
+        }
+    }
+    // the warp that completes the last row-unit of this system folds its partial sums
+    __threadfence();
+    __syncwarp();
+    unsigned int last = 0;
+    if (lane == 0) {
+        const unsigned int prev = atomicAdd(&L.ss[sys].done, (unsigned int)Lr);
+        last = (prev + (unsigned int)Lr == ups) ? 1u : 0u;
+    }
+    last = __shfl_sync(0xffffffffu, last, 0);
+    if (last) {
+        __threadfence();
+        fold_sweep(L, sys, n_strips, k, S);
+    }
+}
+
+// BUDGETS: some system has a step budget (n_steps_total > 0) => the active set is compacted on the fly.
+template <int S, int K, bool BUDGETS>
+__global__ void __launch_bounds__(WarpCfg<S, K>::T, 1) warpsweep_kernel(const __grid_constant__ Layout L) {
+    using Cfg = WarpCfg<S, K>;
+    constexpr int W = Cfg::W, WARPS = Cfg::WARPS, T = Cfg::T;
+    static_assert(Cfg::MAX_SPAN == 64 && WARPS <= 16, "WarpShared sizes");
+    extern __shared__ double2 ws_smem[];
+    __shared__ WarpShared sh;
+
+    const int i = threadIdx.x, lane = i & 31;
+    const int warp = uni(i >> 5);
+    const int rows = L.N + 1;
+    const int n_strips = (L.M1 + W - 1) / W;
+    const int n_bands = (n_strips + WARPS - 1) / WARPS;
+    const unsigned ups = (unsigned)n_strips * (unsigned)rows;                 // row-units per system
+    const long long upb = (long long)n_bands * rows;                          // band-rows per system
+
+    const unsigned base = (unsigned)__cvta_generic_to_shared(ws_smem) + (unsigned)warp * (unsigned)Cfg::warp_bytes;
+    const unsigned ring = base, bars = base + (unsigned)Cfg::off_bars;
+    double* tabp = (double*)((char*)ws_smem + (size_t)warp * Cfg::warp_bytes + Cfg::off_tab);
+    double* accs = (double*)((char*)ws_smem + (size_t)warp * Cfg::warp_bytes + Cfg::off_accs);
+    unsigned t_in = 0;
+    if (lane < Cfg::DIN) mbar_init(bars + (unsigned)lane * 8u, 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+
+    // ---- active systems and this CTA's range of band-rows --------------------------------------------
+    long long n_active = L.n_batch;
+    int a_first = 0;
+    long long start, end;
+    if (BUDGETS) {
+        const int q = (L.n_batch + T - 1) / T;            // systems scanned per thread
+        const int s_lo = min(i * q, L.n_batch), s_hi = min(s_lo + q, L.n_batch);
+        int cnt = 0;
+        for (int s = s_lo; s < s_hi; ++s) cnt += sys_active(L, s, S) ? 1 : 0;
+        int incl = cnt;                                   // inclusive scan over the CTA
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        if (lane == 31) sh.scan[warp] = incl;
+        __syncthreads();
+        int base_a = 0, total = 0;
+#pragma unroll
+        for (int w = 0; w < WARPS; ++w) {
+            if (w < warp) base_a += sh.scan[w];
+            total += sh.scan[w];
+        }
+        n_active = total;
+        const long long units = n_active * upb;
+        const long long U = (units + gridDim.x - 1) / gridDim.x;
+        start = min((long long)blockIdx.x * U, units);
+        end = min(start + U, units);
+        if (start < end) {
+            a_first = (int)(start / upb);
+            const int a_last = (int)((end - 1) / upb);
+            int a = base_a + incl - cnt;                  // index of this thread's first active system
+            for (int s = s_lo; s < s_hi; ++s) {
+                if (sys_active(L, s, S)) {
+                    if (a >= a_first && a <= a_last) sh.list[a - a_first] = s;
+                    ++a;
+                }
+            }
+        }
+    } else {
+        const long long units = n_active * upb;
+        const long long U = (units + gridDim.x - 1) / gridDim.x;
+        start = min((long long)blockIdx.x * U, units);
+        end = min(start + U, units);
+    }
+    __syncthreads();   // mbarriers initialised, list visible
+
+    // ---- every warp walks the CTA's range segment by segment: its strip of the band ----------------------
+    long long pos = start;
+    while (pos < end) {
+        const int a = (int)(pos / upb);
+        const int rem = (int)(pos - (long long)a * upb);
+        const int band = rem / rows;
+        const int r0 = rem - band * rows;
+        const int Lr = (int)min((long long)(rows - r0), end - pos);
+        const int sys = BUDGETS ? uni(sh.list[a - a_first]) : a;
+        const int strip = band * WARPS + warp;
+        pos += Lr;
+        if (strip < n_strips) warpsweep_segment<S, K>(L, sys, strip, r0, Lr, n_strips, ups, ring, tabp, bars, accs, t_in);
+    }
+
+    // ---- the last CTA of the launch advances the step counters of all systems that were active --------
+    __threadfence();
+    __syncthreads();
+    if (i == 0) {
+        const unsigned int prev = atomicAdd(L.gctl, 1u);
+        sh.flag = (prev + 1u == gridDim.x) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (sh.flag) {
+        __threadfence();
+        for (int s = i; s < L.n_batch; s += T)
+            if (sys_active(L, s, S)) { L.ss[s].k += S; L.ss[s].buf ^= 1; }
+        if (i == 0) *L.gctl = 0u;
+    }
+}
+
+}  // namespace bte
