@@ -39,6 +39,10 @@
 
 #include "bte_sweep.cuh"
 
+#ifndef BTE_WS_WARPS
+#define BTE_WS_WARPS 12
+#endif
+
 namespace bte {
 
 template <int S, int K>
@@ -48,12 +52,17 @@ struct WarpCfg {
     static constexpr int HALO = NS - 1;         // halo columns on each side of a strip, halo rows of a segment
     static constexpr int COLS = 32 * K;         // columns a warp computes
     static constexpr int W = COLS - 2 * HALO;   // owned columns per strip
-    static constexpr int WARPS = 8;             // warps per CTA = strips per band
+    static constexpr int WARPS = BTE_WS_WARPS;             // warps per CTA = strips per band
     static constexpr int T = 32 * WARPS;
     static constexpr int DIN = 8;               // slots of the HBM input ring
     static constexpr int DPRE = 6;              // rows prefetched ahead (the slot of record t + DPRE was read 2 iterations ago)
     static constexpr int REC = 2 * COLS + 2;    // double2 per record: A = COLS columns, B = COLS + 2 columns, natural order
     static constexpr int MAX_SPAN = 64;         // distinct systems one CTA range may touch
+    // tensor memory: warp w owns the 32 lanes of quadrant w % 4, columns (w / 4) * TM_COLS .. + 2 NS 8 - 1
+    static constexpr int TM_COLS = 128;
+    static constexpr int TM_NEED = ((WARPS + 3) / 4) * TM_COLS;
+    static constexpr int TM_ALLOC = TM_NEED <= 32 ? 32 : TM_NEED <= 64 ? 64 : TM_NEED <= 128 ? 128 : TM_NEED <= 256 ? 256 : 512;
+    static_assert(2 * NS * 4 * K <= TM_COLS && TM_NEED <= 512, "tensor memory budget");
     // shared memory of one warp: input ring | E(t_v) dt/2 at the NV half-step times | mbarriers | reduction slots [S][2][32]
     static constexpr size_t off_tab = (size_t)DIN * REC * 16;
     static constexpr size_t off_bars = off_tab + (size_t)NV * 8;
@@ -69,6 +78,7 @@ struct WarpShared {
     int scan[16];
     int list[64];
     unsigned int flag;
+    unsigned int tmem_base;
 };
 
 __device__ __forceinline__ double2 shfl_up_d2(double2 v) {
@@ -114,6 +124,34 @@ __device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned
                  : "memory");
 }
 
+// ---- tensor memory as the warp's private scratchpad (tcgen05.st / tcgen05.ld, 32 lanes x 32-bit columns) ----
+// A warp reaches the 32 TMEM lanes of its quadrant (warp % 4); the partial right-hand sides of the rows in flight live
+// there instead of in registers (96 registers per thread at S = 3).  Measured on B200 (one SM): 744 B/clk loads,
+// 1000 B/clk stores, 39 cycles load-to-use -- 6 x the shared-memory bandwidth, on a path of its own.
+// one double per store: its register pair is the natural operand (wider stores want 4 or 8 consecutive registers,
+// which ptxas gathers with moves)
+__device__ __forceinline__ void tm_st_d(unsigned taddr, double a) {
+    asm volatile("{\n .reg .b32 lo, hi;\n mov.b64 {lo, hi}, %1;\n tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {lo, hi};\n}\n" ::"r"(taddr), "d"(a)
+                 : "memory");
+}
+__device__ __forceinline__ void tm_st_d2(unsigned taddr, double2 a) {
+    tm_st_d(taddr, a.x);
+    tm_st_d(taddr + 2u, a.y);
+}
+__device__ __forceinline__ void tm_ld_x8(unsigned taddr, unsigned (&r)[8]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr)
+                 : "memory");
+}
+// the loaded registers may be read only after the wait: the wait takes them as in/out operands so that no use can be
+// scheduled above it
+__device__ __forceinline__ void tm_wait_ld(unsigned (&r)[8]) {
+    asm volatile("tcgen05.wait::ld.sync.aligned;\n"
+                 : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7])::"memory");
+}
+__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;\n" ::: "memory"); }
+
 __device__ __forceinline__ bool elect_one() {
     unsigned ok;
     asm volatile("{\n .reg .pred p;\n elect.sync _|p, 0xffffffff;\n selp.u32 %0, 1, 0, p;\n}\n" : "=r"(ok));
@@ -133,7 +171,7 @@ template <int S, int K>
 __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys, const int strip, const int r0,
                                                   const int Lr, const int n_strips, const unsigned ups,
                                                   const unsigned ring, double* tabp, const unsigned bars,
-                                                  double* __restrict__ accs, unsigned& t_in) {
+                                                  const unsigned tmP, double* __restrict__ accs, unsigned& t_in) {
     using Cfg = WarpCfg<S, K>;
     constexpr int NS = Cfg::NS, NV = Cfg::NV, HALO = Cfg::HALO, W = Cfg::W, REC = Cfg::REC;
     constexpr int DIN = Cfg::DIN, DPRE = Cfg::DPRE;
@@ -198,19 +236,17 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
     __syncwarp();
     // Rows outside the lattice / the trapezoid are clamped to the nearest row the segment reads anyway (the record is
     // then read as zero, see `okh`, `okf` below): the prefetch is branch-free, two copies of fixed size per record.
-    const double2* gA = Hin + (min(max(rpre + 2, 0), rh_max) * pitch + ca0);
-    const double2* gF = Hin + (Y + min(max(rpre + 1, 0), rf_max) * pitch + cb0);
+    const double2* gA = Hin + ca0;
+    const double2* gF = Hin + (Y + cb0);
     auto prefetch = [&]() {
         // (the record that lived in this slot was read two iterations ago: those loads have long been consumed)
         if (rpre <= rho_end && elect_one()) {
             const unsigned slot = tpre & (DIN - 1);
             const unsigned dst = ring + slot * RB, bar = bars + slot * 8;
             mbar_arrive_expect_tx(bar, nA + nB);
-            bulk_g2s(dst + dA, gA, nA, bar);
-            bulk_g2s(dst + dB, gF, nB, bar);
+            bulk_g2s(dst + dA, gA + min(max(rpre + 2, 0), rh_max) * pitch, nA, bar);
+            bulk_g2s(dst + dB, gF + min(max(rpre + 1, 0), rf_max) * pitch, nB, bar);
         }
-        if (rpre + 2 >= 0 && rpre + 2 < rh_max) gA += pitch;
-        if (rpre + 1 >= 0 && rpre + 1 < rf_max) gF += pitch;
         ++tpre; ++rpre;
     };
 #pragma unroll
@@ -221,22 +257,24 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
     double2* __restrict__ Hout = state_ptr(L, nxt, 0, sys) + col0;
     double2* __restrict__ Fout = Hout + Y;
 
-    double2 P[NS][2][K];                                // partial right-hand sides in flight: [stage][slot][column]
+    // partial right-hand sides in flight: tensor memory, [stage][slot] x (K pairs = 8 columns of 32 bits); the slot
+    // is the parity of the iteration (a row started in iteration rho is finished in iteration rho + 2)
+    static_assert(K == 2, "one x8 tensor-memory access holds the K = 2 pairs of a stage");
 #pragma unroll
-    for (int j = 0; j < NS; ++j)
-#pragma unroll
-        for (int q = 0; q < K; ++q) P[j][0][q] = P[j][1][q] = zero;
+    for (int e = 0; e < 4 * NS; ++e) tm_st_d2(tmP + (unsigned)e * 4u, zero);
 
     int rho = rho_start;
     double nd0 = (double)rho;                           // row finished by stage 0, as double
     int o_out = (rho - (NS - 2)) * pitch;               // element offset of the row finished by stage NS - 2
     const double* cnp = cn0 + (rho + 2);                // c_n of the row started by stage 0 (stage j: j rows back)
+    unsigned tmS = tmP;                                 // tensor-memory address of stage 0's slot of this iteration
 
-    // edge_tag: std::true_type = fill / drain iteration (row predicates, special rows 0 and 1);
-    // par_tag: steady state only: which of the two slots of P is finished (and refilled) in this iteration
-    auto body = [&](auto edge_tag, auto par_tag) {
+    // edge_tag: std::true_type = fill / drain iteration (row predicates, special rows 0 and 1)
+    auto body = [&](auto edge_tag) {
         constexpr bool EDGE = decltype(edge_tag)::value;
-        constexpr int PAR = decltype(par_tag)::value;
+        tm_wait_st();                                   // the partial sums stored in the previous iterations are in place
+        unsigned Praw[8];
+        tm_ld_x8(tmS, Praw);                            // stage 0's rows in flight
         // ---- take record rho ----
         double2 Z[NS + 2][K];                           // Z[j + 2] = output of stage j; Z[0] = A, Z[1] = B
         double2 FL, FR;                                 // F^0 columns left / right of this lane's K columns
@@ -294,81 +332,73 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
 #pragma unroll
                 for (int q = 0; q < K; ++q) pq[j + 1 < NS ? j + 1 : 0][q] = cn_coef(mu[j + 3][q], L.nu, L.nu2);
             }
-            if (!EDGE || comp || strt) {
-                double2 D[K];
+            // this stage's rows in flight have arrived; ask for the next stage's
+            tm_wait_ld(Praw);
+            double2 Pq[K];
+#pragma unroll
+            for (int q = 0; q < K; ++q) {
+                Pq[q].x = __hiloint2double((int)Praw[4 * q + 1], (int)Praw[4 * q]);
+                Pq[q].y = __hiloint2double((int)Praw[4 * q + 3], (int)Praw[4 * q + 2]);
+            }
+            if (j + 1 < NS) tm_ld_x8(tmS + (unsigned)(j + 1) * 16u, Praw);
+            double2 D[K];
+#pragma unroll
+            for (int q = 0; q < K; ++q) {
+                const double2 r = (q + 1 < K) ? src[q + 1 < K ? q + 1 : 0] : Rv;
+                const double2 l = (q > 0) ? src[q > 0 ? q - 1 : 0] : Lv;
+                D[q].x = __dsub_rn(r.x, l.x);
+                D[q].y = __dsub_rn(r.y, l.y);
+            }
+            if (comp) {
 #pragma unroll
                 for (int q = 0; q < K; ++q) {
-                    const double2 r = (q + 1 < K) ? src[q + 1 < K ? q + 1 : 0] : Rv;
-                    const double2 l = (q > 0) ? src[q > 0 ? q - 1 : 0] : Lv;
-                    D[q].x = __dsub_rn(r.x, l.x);
-                    D[q].y = __dsub_rn(r.y, l.y);
+                    Zo[q] = cn_apply(Pq[q], D[q], kap[q], pq[j][q]);
+                    if (EDGE && n == 0) Zo[q].y = 0.0;                // b_0 == 0 (eq. 23, C3)
                 }
-                if (comp) {
+                const bool mine = !EDGE || (n >= r0 && n < r0 + Lr);
+                if (j >= NS - 2 && mine) {                            // the two newest time levels go to HBM
+                    double2* out = (j == NS - 1) ? Fout + (o_out - pitch) : Hout + o_out;
 #pragma unroll
-                    for (int q = 0; q < K; ++q) {
-                        const double2 Pq = EDGE ? P[j][0][q] : P[j][PAR][q];
-                        Zo[q] = cn_apply(Pq, D[q], kap[q], pq[j][q]);
-                        if (EDGE && n == 0) Zo[q].y = 0.0;            // b_0 == 0 (eq. 23, C3)
-                    }
-                    const bool mine = !EDGE || (n >= r0 && n < r0 + Lr);
-                    if (j >= NS - 2 && mine) {                        // the two newest time levels go to HBM
-                        double2* out = (j == NS - 1) ? Fout + (o_out - pitch) : Hout + o_out;
+                    for (int q = 0; q < K; ++q)
+                        if (own[q]) out[q] = Zo[q];
+                }
+                if (EDGE && (j & 1) == 0 && mine && n <= 1) {         // whole grid of step k + j/2 + 1: reductions
+                    double v = 0.0;
 #pragma unroll
-                        for (int q = 0; q < K; ++q)
-                            if (own[q]) out[q] = Zo[q];
-                    }
-                    if (EDGE && (j & 1) == 0 && mine && n <= 1) {     // whole grid of step k + j/2 + 1: reductions
-                        double v = 0.0;
+                    for (int q = 0; q < K; ++q)
+                        if (own[q]) v += (n == 0) ? Zo[q].x : Zo[q].y;
+                    accs[((j >> 1) * 2 + n) * 32 + lane] = v;
+                    if (j == NS - 2 && n == 1) {
 #pragma unroll
-                        for (int q = 0; q < K; ++q)
-                            if (own[q]) v += (n == 0) ? Zo[q].x : Zo[q].y;
-                        accs[((j >> 1) * 2 + n) * 32 + lane] = v;
-                        if (j == NS - 2 && n == 1) {
-#pragma unroll
-                            for (int q = 0; q < K; ++q) {
-                                if (own[q] && col0 + q == 0) L.ss[sys].edge[0] = fabs(Zo[q].y);
-                                if (own[q] && col0 + q == L.M1 - 1) L.ss[sys].edge[1] = fabs(Zo[q].y);
-                            }
+                        for (int q = 0; q < K; ++q) {
+                            if (own[q] && col0 + q == 0) L.ss[sys].edge[0] = fabs(Zo[q].y);
+                            if (own[q] && col0 + q == L.M1 - 1) L.ss[sys].edge[1] = fabs(Zo[q].y);
                         }
-                    }
-                } else {
-#pragma unroll
-                    for (int q = 0; q < K; ++q) Zo[q] = zero;         // outside the lattice / this segment's halo
-                }
-                if (EDGE) {
-#pragma unroll
-                    for (int q = 0; q < K; ++q) P[j][0][q] = P[j][1][q];
-                }
-                if (strt) {
-                    const double cj = __ldg(cnp - j);                 // c_{n+2}
-#pragma unroll
-                    for (int q = 0; q < K; ++q) {
-                        double2 lo = D[q];
-                        if (EDGE && n + 2 == 1) lo.x *= 2.0;          // chi(1) = 2, eq. (11)
-                        const double2 Pn = cn_partial(ownp[q], lo, mu[j][q], __dmul_rn(cj, gdt[q]), kap[q], L.xi);
-                        if (EDGE) P[j][1][q] = Pn; else P[j][PAR][q] = Pn;
                     }
                 }
             } else {
 #pragma unroll
+                for (int q = 0; q < K; ++q) Zo[q] = zero;             // outside the lattice / this segment's halo
+            }
+            if (strt) {
+                const double cj = __ldg(cnp - j);                     // c_{n+2}
+#pragma unroll
                 for (int q = 0; q < K; ++q) {
-                    Zo[q] = zero;
-                    P[j][0][q] = P[j][1][q];
+                    double2 lo = D[q];
+                    if (EDGE && n + 2 == 1) lo.x *= 2.0;              // chi(1) = 2, eq. (11)
+                    const double2 Pn = cn_partial(ownp[q], lo, mu[j][q], __dmul_rn(cj, gdt[q]), kap[q], L.xi);
+                    tm_st_d2(tmS + (unsigned)(j * 16 + q * 4), Pn);   // finished two iterations from now
                 }
             }
         }
         ++rho; nd0 += 1.0;
         o_out += pitch; ++cnp;
+        tmS ^= 8u;                                      // the other slot
     };
 
-    using P0 = std::integral_constant<int, 0>;
-    using P1 = std::integral_constant<int, 1>;
-    while (rho <= rho_end && rho < rho_s0) body(std::true_type{}, P0{});
-    while (rho + 1 <= rho_s1) {                         // two iterations per trip: the slots of P alternate
-        body(std::false_type{}, P0{});
-        body(std::false_type{}, P1{});
-    }
-    while (rho <= rho_end) body(std::true_type{}, P0{});
+    while (rho <= rho_end && rho < rho_s0) body(std::true_type{});
+    while (rho <= rho_s1) body(std::false_type{});
+    while (rho <= rho_end) body(std::true_type{});
 
     // per-strip partial sums of row 0 (a) and row 1 (b) of the S new whole grids -> eq. (12), (20)
     const bool has0 = (r0 == 0), has1 = (r0 <= 1) && (r0 + Lr > 1);
@@ -426,6 +456,12 @@ __global__ void __launch_bounds__(WarpCfg<S, K>::T, 1) warpsweep_kernel(const __
     unsigned t_in = 0;
     if (lane < Cfg::DIN) mbar_init(bars + (unsigned)lane * 8u, 1u);
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    if (warp == 0) {                                      // one CTA per SM (launch bounds, shared memory): no contention
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(
+                         (unsigned)__cvta_generic_to_shared(&sh.tmem_base)), "r"(Cfg::TM_ALLOC) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
 
     // ---- active systems and this CTA's range of band-rows --------------------------------------------
     long long n_active = L.n_batch;
@@ -472,7 +508,9 @@ __global__ void __launch_bounds__(WarpCfg<S, K>::T, 1) warpsweep_kernel(const __
         start = min((long long)blockIdx.x * U, units);
         end = min(start + U, units);
     }
-    __syncthreads();   // mbarriers initialised, list visible
+    __syncthreads();   // mbarriers initialised, list visible, tensor memory allocated
+    asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+    const unsigned tmP = uni(sh.tmem_base) + (((unsigned)(warp & 3) * 32u) << 16) + (unsigned)(warp >> 2) * Cfg::TM_COLS;
 
     // ---- every warp walks the CTA's range segment by segment: its strip of the band ----------------------
     long long pos = start;
@@ -485,12 +523,16 @@ __global__ void __launch_bounds__(WarpCfg<S, K>::T, 1) warpsweep_kernel(const __
         const int sys = BUDGETS ? uni(sh.list[a - a_first]) : a;
         const int strip = band * WARPS + warp;
         pos += Lr;
-        if (strip < n_strips) warpsweep_segment<S, K>(L, sys, strip, r0, Lr, n_strips, ups, ring, tabp, bars, accs, t_in);
+        if (strip < n_strips) warpsweep_segment<S, K>(L, sys, strip, r0, Lr, n_strips, ups, ring, tabp, bars, tmP, accs, t_in);
     }
 
     // ---- the last CTA of the launch advances the step counters of all systems that were active --------
+    tm_wait_st();
+    asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
     __threadfence();
     __syncthreads();
+    if (warp == 0)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(sh.tmem_base), "r"(Cfg::TM_ALLOC) : "memory");
     if (i == 0) {
         const unsigned int prev = atomicAdd(L.gctl, 1u);
         sh.flag = (prev + 1u == gridDim.x) ? 1u : 0u;
