@@ -238,7 +238,7 @@ constexpr int WS_MAX_STEPS = 3;     // the register-resident kernel is instantia
 static_assert(WS_MAX_STEPS <= SWEEP_MAX_STEPS, "partial sums are laid out for SWEEP_MAX_STEPS steps per pass");
 
 // register-resident warp kernel (bte_warpsweep.cuh): S = 2, 3 steps per pass, K = 2 columns per lane
-constexpr int RS_K = 2;
+constexpr int RS_K = BTE_WS_K;
 template <int S>
 SweepFn regsweep_fn_s(bool budgets) {
     using Cfg = WarpCfg<S, RS_K>;

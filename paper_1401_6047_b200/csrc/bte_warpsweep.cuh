@@ -40,7 +40,16 @@
 #include "bte_sweep.cuh"
 
 #ifndef BTE_WS_WARPS
-#define BTE_WS_WARPS 12
+#define BTE_WS_WARPS 8
+#endif
+#ifndef BTE_WS_K
+#define BTE_WS_K 3
+#endif
+#ifndef BTE_WS_DIN
+#define BTE_WS_DIN 8
+#endif
+#ifndef BTE_WS_CG
+#define BTE_WS_CG 3
 #endif
 
 namespace bte {
@@ -54,15 +63,18 @@ struct WarpCfg {
     static constexpr int W = COLS - 2 * HALO;   // owned columns per strip
     static constexpr int WARPS = BTE_WS_WARPS;             // warps per CTA = strips per band
     static constexpr int T = 32 * WARPS;
-    static constexpr int DIN = 8;               // slots of the HBM input ring
-    static constexpr int DPRE = 6;              // rows prefetched ahead (the slot of record t + DPRE was read 2 iterations ago)
+    static constexpr int DIN = BTE_WS_DIN;      // slots of the HBM input ring
+    static constexpr int DPRE = DIN - 2;              // rows prefetched ahead (the slot of record t + DPRE was read 2 iterations ago)
     static constexpr int REC = 2 * COLS + 2;    // double2 per record: A = COLS columns, B = COLS + 2 columns, natural order
+    static constexpr int CG = BTE_WS_CG < 2 * S ? BTE_WS_CG : 2 * S;   // stages whose coefficients are formed together
     static constexpr int MAX_SPAN = 64;         // distinct systems one CTA range may touch
-    // tensor memory: warp w owns the 32 lanes of quadrant w % 4, columns (w / 4) * TM_COLS .. + 2 NS 8 - 1
-    static constexpr int TM_COLS = 128;
+    // tensor memory: warp w owns the 32 lanes of quadrant w % 4, columns (w / 4) * TM_COLS .. + 2 NS TM_SLOT - 1;
+    // one slot = the K pairs (4 K 32-bit columns, rounded to a power of two) of one stage and one iteration parity
+    static constexpr int TM_SLOT = K <= 2 ? 8 : 16;
+    static constexpr int TM_COLS = 2 * NS * TM_SLOT;
     static constexpr int TM_NEED = ((WARPS + 3) / 4) * TM_COLS;
     static constexpr int TM_ALLOC = TM_NEED <= 32 ? 32 : TM_NEED <= 64 ? 64 : TM_NEED <= 128 ? 128 : TM_NEED <= 256 ? 256 : 512;
-    static_assert(2 * NS * 4 * K <= TM_COLS && TM_NEED <= 512, "tensor memory budget");
+    static_assert(4 * K <= TM_SLOT && TM_NEED <= 512, "tensor memory budget");
     // shared memory of one warp: input ring | E(t_v) dt/2 at the NV half-step times | mbarriers | reduction slots [S][2][32]
     static constexpr size_t off_tab = (size_t)DIN * REC * 16;
     static constexpr size_t off_bars = off_tab + (size_t)NV * 8;
@@ -138,17 +150,34 @@ __device__ __forceinline__ void tm_st_d2(unsigned taddr, double2 a) {
     tm_st_d(taddr, a.x);
     tm_st_d(taddr + 2u, a.y);
 }
-__device__ __forceinline__ void tm_ld_x8(unsigned taddr, unsigned (&r)[8]) {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
-                 : "r"(taddr)
-                 : "memory");
+template <int NR>
+__device__ __forceinline__ void tm_ld(unsigned taddr, unsigned (&r)[NR]) {
+    static_assert(NR == 8 || NR == 16, "x8 or x16");
+    if constexpr (NR == 8) {
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n"
+                     : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                     : "r"(taddr)
+                     : "memory");
+    } else {
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];\n"
+                     : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+                       "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+                     : "r"(taddr)
+                     : "memory");
+    }
 }
 // the loaded registers may be read only after the wait: the wait takes them as in/out operands so that no use can be
 // scheduled above it
-__device__ __forceinline__ void tm_wait_ld(unsigned (&r)[8]) {
-    asm volatile("tcgen05.wait::ld.sync.aligned;\n"
-                 : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7])::"memory");
+template <int NR>
+__device__ __forceinline__ void tm_wait_ld(unsigned (&r)[NR]) {
+    if constexpr (NR == 8) {
+        asm volatile("tcgen05.wait::ld.sync.aligned;\n"
+                     : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7])::"memory");
+    } else {
+        asm volatile("tcgen05.wait::ld.sync.aligned;\n"
+                     : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]),
+                       "+r"(r[8]), "+r"(r[9]), "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15])::"memory");
+    }
 }
 __device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;\n" ::: "memory"); }
 
@@ -259,9 +288,9 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
 
     // partial right-hand sides in flight: tensor memory, [stage][slot] x (K pairs = 8 columns of 32 bits); the slot
     // is the parity of the iteration (a row started in iteration rho is finished in iteration rho + 2)
-    static_assert(K == 2, "one x8 tensor-memory access holds the K = 2 pairs of a stage");
+    constexpr int SL = Cfg::TM_SLOT;
 #pragma unroll
-    for (int e = 0; e < 4 * NS; ++e) tm_st_d2(tmP + (unsigned)e * 4u, zero);
+    for (int e = 0; e < 2 * NS * SL / 4; ++e) tm_st_d2(tmP + (unsigned)e * 4u, zero);
 
     int rho = rho_start;
     double nd0 = (double)rho;                           // row finished by stage 0, as double
@@ -272,9 +301,11 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
     // edge_tag: std::true_type = fill / drain iteration (row predicates, special rows 0 and 1)
     auto body = [&](auto edge_tag) {
         constexpr bool EDGE = decltype(edge_tag)::value;
+#ifndef BTE_NO_WAIT_ST
         tm_wait_st();                                   // the partial sums stored in the previous iterations are in place
-        unsigned Praw[8];
-        tm_ld_x8(tmS, Praw);                            // stage 0's rows in flight
+#endif
+        unsigned Praw[SL];
+        tm_ld(tmS, Praw);                            // stage 0's rows in flight
         // ---- take record rho ----
         double2 Z[NS + 2][K];                           // Z[j + 2] = output of stage j; Z[0] = A, Z[1] = B
         double2 FL, FR;                                 // F^0 columns left / right of this lane's K columns
@@ -302,12 +333,20 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
 #pragma unroll
             for (int q = 0; q < K; ++q) mu[v][q] = __fma_rn(ndv, bph[q], ndE);
         };
+        // coefficients: they depend on (row, column, time) only, so the reciprocal chains are independent of each other
+        // and of the data; they are formed for CG stages at a time (CG K independent chains side by side)
         form_mu(0);
         form_mu(1);
-        form_mu(2);
-        double2 pq[NS][K];                              // (nu, mu') / (nu^2 + mu'^2) of stage j: formed one stage ahead
+        double2 pq[NS][K];                              // (nu, mu') / (nu^2 + mu'^2) of stage j
+        auto form_coef = [&](const int j0) {
 #pragma unroll
-        for (int q = 0; q < K; ++q) pq[0][q] = cn_coef(mu[2][q], L.nu, L.nu2);
+            for (int j = j0; j < j0 + Cfg::CG && j < NS; ++j) form_mu(j + 2);
+#pragma unroll
+            for (int j = j0; j < j0 + Cfg::CG && j < NS; ++j)
+#pragma unroll
+                for (int q = 0; q < K; ++q) pq[j][q] = cn_coef(mu[j + 2][q], L.nu, L.nu2);
+        };
+        form_coef(0);
 #pragma unroll
         for (int j = 0; j < NS; ++j) {
             // src = Z[j + 1] = row n + 1 of the stencil grid X^j, ownp = Z[j] = own pairs of row n + 2;
@@ -327,11 +366,7 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
             double2 Lv, Rv;
             if (j == 0) { Lv = FL; Rv = FR; }
             else { Lv = shfl_up_d2(src[K - 1]); Rv = shfl_down_d2(src[0]); }
-            if (j + 1 < NS) {                                         // coefficients of the next stage: independent of
-                form_mu(j + 3);                                       // the data, they fill the latency of the shuffles
-#pragma unroll
-                for (int q = 0; q < K; ++q) pq[j + 1 < NS ? j + 1 : 0][q] = cn_coef(mu[j + 3][q], L.nu, L.nu2);
-            }
+            if ((j + 1) % Cfg::CG == 0 && j + 1 < NS) form_coef(j + 1);   // while the shuffles are in flight
             // this stage's rows in flight have arrived; ask for the next stage's
             tm_wait_ld(Praw);
             double2 Pq[K];
@@ -340,7 +375,7 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
                 Pq[q].x = __hiloint2double((int)Praw[4 * q + 1], (int)Praw[4 * q]);
                 Pq[q].y = __hiloint2double((int)Praw[4 * q + 3], (int)Praw[4 * q + 2]);
             }
-            if (j + 1 < NS) tm_ld_x8(tmS + (unsigned)(j + 1) * 16u, Praw);
+            if (j + 1 < NS) tm_ld(tmS + (unsigned)((j + 1) * 2 * SL), Praw);
             double2 D[K];
 #pragma unroll
             for (int q = 0; q < K; ++q) {
@@ -387,13 +422,13 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
                     double2 lo = D[q];
                     if (EDGE && n + 2 == 1) lo.x *= 2.0;              // chi(1) = 2, eq. (11)
                     const double2 Pn = cn_partial(ownp[q], lo, mu[j][q], __dmul_rn(cj, gdt[q]), kap[q], L.xi);
-                    tm_st_d2(tmS + (unsigned)(j * 16 + q * 4), Pn);   // finished two iterations from now
+                    tm_st_d2(tmS + (unsigned)(j * 2 * SL + q * 4), Pn);   // finished two iterations from now
                 }
             }
         }
         ++rho; nd0 += 1.0;
         o_out += pitch; ++cnp;
-        tmS ^= 8u;                                      // the other slot
+        tmS ^= (unsigned)SL;                            // the other slot
     };
 
     while (rho <= rho_end && rho < rho_s0) body(std::true_type{});
