@@ -39,7 +39,7 @@ BYTES_PER_UPDATE = 64.0       # a_h, b_h, a_f, b_f each read once and written on
 FP64_PER_HALF_UPDATE = 23     # cn_partial + cn_complete + differences, src, mu (bte_device.cuh)
 FP64_PEAK_INSTR = 148 * 64 * 1.965e9   # DFMA-class thread-instructions/s: 148 SMs x 64 lanes x max SM clock
 VARIANT_KERNEL = {1: "half_update_kernel (two launches per step)", 2: "fused_step_kernel", 3: "sweep_kernel",
-                  5: "regsweep_kernel"}
+                  5: "warpsweep_kernel"}
 VARIANT_BYTES = {1: 96.0, 2: 64.0, 3: 64.0, 5: 64.0}   # HBM bytes per lattice point and launch group
 
 
@@ -60,8 +60,8 @@ def recorded_traffic(workload_name, kernel, steps_per_launch):
             d = json.load(f)
         e = d.get(workload_name, {})
         key = f"S{int(round(steps_per_launch))}"
-        if kernel.startswith("regsweep"):
-            key = "reg" + key
+        if kernel.startswith("warpsweep"):
+            key = "warp" + key
         return e.get(key, {}).get("dram_bytes_per_launch")
     except Exception:
         return None

@@ -128,7 +128,7 @@ void bessel_i_ratios(double x, int N, std::vector<double>& r) {
     for (int n = 0; n <= N; ++n) r[n] = t[n] / t[0];
 }
 
-enum Variant { VAR_AUTO = 0, VAR_SPLIT = 1, VAR_FUSED = 2, VAR_SWEEP = 3, VAR_RESIDENT = 4, VAR_REGSWEEP = 5 };
+enum Variant { VAR_AUTO = 0, VAR_SPLIT = 1, VAR_FUSED = 2, VAR_SWEEP = 3, VAR_RESIDENT = 4, VAR_WARPSWEEP = 5 };
 
 }  // namespace
 
@@ -155,8 +155,7 @@ struct bte_ctx {
     int sweep_ctas;                  // option: grid-size override (0 = SMs x resident CTAs)
     int sweep_threads;               // option: 0 = automatic, 128, 256
     int sw_grid[SWEEP_MAX_STEPS + 1];   // grid of the S-step kernel; 0 = not usable for this problem
-    int rs_grid[SWEEP_MAX_STEPS + 1];   // same for the register-pipelined kernel (bte_regsweep.cuh), S >= 2
-    int rs_cols;                     // option: columns per lane of the register-pipelined kernel (0 = automatic)
+    int ws_grid[SWEEP_MAX_STEPS + 1];   // same for the warp kernel (bte_warpsweep.cuh), S = 2 .. WS_MAX_STEPS
     int sm_count;
     std::vector<int64_t> budgets;    // sorted distinct step budgets (n_steps_total > 0)
     // resident (on-chip) kernel launch plan
@@ -234,21 +233,22 @@ SweepFn sweep_fn(int S, bool budgets, int wide) {
     }
 }
 constexpr int RING_MAX_STEPS = 3;   // the shared-memory-ring kernel is instantiated for S = 1 .. 3
+constexpr int WARP_MIN_ROWS = 96;   // automatic choice of the warp kernel: columns at least this long (measured: config 3, 41 rows, is faster on the ring kernel)
 constexpr int WS_MAX_STEPS = 3;     // the register-resident kernel is instantiated for S = 2, 3
 static_assert(WS_MAX_STEPS <= SWEEP_MAX_STEPS, "partial sums are laid out for SWEEP_MAX_STEPS steps per pass");
 
-// register-resident warp kernel (bte_warpsweep.cuh): S = 2, 3 steps per pass, K = 2 columns per lane
-constexpr int RS_K = BTE_WS_K;
+// register-resident warp kernel (bte_warpsweep.cuh): S = 2, 3 steps per pass, K = BTE_WS_K columns per lane
+constexpr int WS_K = BTE_WS_K;
 template <int S>
-SweepFn regsweep_fn_s(bool budgets) {
-    using Cfg = WarpCfg<S, RS_K>;
-    return {budgets ? (void*)warpsweep_kernel<S, RS_K, true> : (void*)warpsweep_kernel<S, RS_K, false>,
+SweepFn warpsweep_fn_s(bool budgets) {
+    using Cfg = WarpCfg<S, WS_K>;
+    return {budgets ? (void*)warpsweep_kernel<S, WS_K, true> : (void*)warpsweep_kernel<S, WS_K, false>,
             Cfg::smem_bytes, Cfg::W, Cfg::T, Cfg::WARPS};
 }
-SweepFn regsweep_fn(int S, bool budgets) {
+SweepFn warpsweep_fn(int S, bool budgets) {
     switch (S) {
-        case 2: return regsweep_fn_s<2>(budgets);
-        default: return regsweep_fn_s<3>(budgets);
+        case 2: return warpsweep_fn_s<2>(budgets);
+        default: return warpsweep_fn_s<3>(budgets);
     }
 }
 
@@ -262,16 +262,16 @@ int sweep_wide(const bte_ctx* c, int S) {
 }
 
 int plan_sweep(bte_ctx* c) {
-    for (int S = 0; S <= SWEEP_MAX_STEPS; ++S) c->sw_grid[S] = c->rs_grid[S] = 0;
+    for (int S = 0; S <= SWEEP_MAX_STEPS; ++S) c->sw_grid[S] = c->ws_grid[S] = 0;
     if (c->grid.precision != 0) return BTE_OK;     // fp32 variants run the split kernels only
     int dev = 0, sms = 0;
     CUDA_TRY(cudaGetDevice(&dev));
     CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     c->sm_count = sms;
     const long long rows_alloc = c->grid.n_harm + 1 + 2 * GHOST;
-    // register-pipelined kernel: one CTA (teams of S warps) per SM; a CTA range is counted in band-rows
+    // warp kernel: one CTA of WARPS independent warps per SM; a CTA range is counted in band-rows
     for (int S = 2; S <= WS_MAX_STEPS; ++S) {
-        const SweepFn f = regsweep_fn(S, c->has_budgets);
+        const SweepFn f = warpsweep_fn(S, c->has_budgets);
         int occ = 0;
         cudaError_t e = cudaFuncSetAttribute(f.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f.smem);
         if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f.fn, f.T, f.smem);
@@ -290,8 +290,8 @@ int plan_sweep(bte_ctx* c) {
         if (c->sweep_ctas > 0) g = c->sweep_ctas;
         if (g > (units + min_rows - 1) / min_rows) g = (units + min_rows - 1) / min_rows;
         if (g < 1) g = 1;
-        if (c->has_budgets && (long long)c->grid.n_batch / g + 2 > WarpCfg<2, RS_K>::MAX_SPAN) continue;
-        c->rs_grid[S] = (int)g;
+        if (c->has_budgets && (long long)c->grid.n_batch / g + 2 > WarpCfg<2, WS_K>::MAX_SPAN) continue;
+        c->ws_grid[S] = (int)g;
     }
     for (int S = 1; S <= RING_MAX_STEPS; ++S) {
         c->sw_grid[S] = 0;
@@ -437,20 +437,25 @@ int launch_resident(bte_ctx* c, int64_t n_steps) {
 
 int effective_variant(const bte_ctx* c) {
     if (c->grid.precision != 0) return VAR_SPLIT;
-    if (c->variant == VAR_REGSWEEP && c->sw_grid[1] > 0 && c->rs_grid[2] > 0) return VAR_REGSWEEP;
-    // AUTO, and what runs when the resident kernel is not used: the shared-memory-ring sweep kernel
-    const bool streaming = c->variant == VAR_AUTO || c->variant == VAR_RESIDENT || c->variant == VAR_REGSWEEP;
+    // one-step launches of the warp kernel's plan run the ring kernel (the HBM-bound form), so both must be usable
+    const bool warp_ok = c->sw_grid[1] > 0 && c->ws_grid[2] > 0;
+    if (c->variant == VAR_WARPSWEEP && warp_ok) return VAR_WARPSWEEP;
+    // AUTO, and what runs when the resident kernel is not used: a streaming kernel.  Long columns: the warp kernel
+    // (registers + tensor memory; a segment costs 3 NS extra row iterations, so it wants a long march over n); short
+    // columns (batches of small systems): the shared-memory-ring kernel at S = 2.
+    const bool streaming = c->variant == VAR_AUTO || c->variant == VAR_RESIDENT || c->variant == VAR_WARPSWEEP;
+    if (streaming && warp_ok && c->ws_grid[WS_MAX_STEPS] > 0 && c->grid.n_harm + 1 >= WARP_MIN_ROWS) return VAR_WARPSWEEP;
     if (streaming || c->variant == VAR_SWEEP) return c->sw_grid[1] > 0 ? VAR_SWEEP : VAR_FUSED;
     return c->variant;
 }
 
-bool is_sweep(int var) { return var == VAR_SWEEP || var == VAR_REGSWEEP; }
+bool is_sweep(int var) { return var == VAR_SWEEP || var == VAR_WARPSWEEP; }
 
 // is an s-step launch available in the effective streaming variant?  (one-step launches always run the
 // shared-memory-ring kernel: the HBM-bound form, bte_sweep.cuh)
 bool sweep_has(const bte_ctx* c, int var, int s) {
     if (s == 1) return c->sw_grid[1] > 0;
-    return var == VAR_REGSWEEP ? c->rs_grid[s] > 0 : (s <= RING_MAX_STEPS && c->sw_grid[s] > 0);
+    return var == VAR_WARPSWEEP ? c->ws_grid[s] > 0 : (s <= RING_MAX_STEPS && c->sw_grid[s] > 0);
 }
 
 // steps fused per launch by the sweep kernels (the other variants advance one step per launch group)
@@ -458,7 +463,7 @@ int sweep_steps(const bte_ctx* c) {
     const int var = effective_variant(c);
     if (!is_sweep(var)) return 1;
     int S;
-    if (var == VAR_REGSWEEP) {
+    if (var == VAR_WARPSWEEP) {
         S = c->sweep_steps > 0 ? c->sweep_steps : 3;
     } else {
         // ring kernel: 3 steps per pass when the march over n is long enough to amortise the 3 NS - 1
@@ -471,9 +476,9 @@ int sweep_steps(const bte_ctx* c) {
 
 // kernel, launch shape and grid of an s-step launch of the effective streaming variant
 SweepFn sweep_launch(const bte_ctx* c, int var, int s, int* grid) {
-    if (var == VAR_REGSWEEP && s >= 2) {
-        *grid = c->rs_grid[s];
-        return regsweep_fn(s, c->has_budgets);
+    if (var == VAR_WARPSWEEP && s >= 2) {
+        *grid = c->ws_grid[s];
+        return warpsweep_fn(s, c->has_budgets);
     }
     *grid = c->sw_grid[s];
     return sweep_fn(s, c->has_budgets, sweep_wide(c, s));
@@ -718,8 +723,7 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
     c->budgets.erase(std::unique(c->budgets.begin(), c->budgets.end()), c->budgets.end());
     c->sweep_steps = 0; c->sweep_ctas = 0; c->sm_count = 0; c->graph_S = 0; c->sweep_threads = 0;
     c->res_ctas_opt = 0; c->res_mode = -1; c->res_G = 0; c->res_Wc = 0; c->res_T = 0; c->res_smem = 0;
-    for (int S = 0; S <= SWEEP_MAX_STEPS; ++S) c->sw_grid[S] = c->rs_grid[S] = 0;
-    c->rs_cols = 0;
+    for (int S = 0; S <= SWEEP_MAX_STEPS; ++S) c->sw_grid[S] = c->ws_grid[S] = 0;
     c->steps_issued = 0; c->launches = 0;
     c->variant = VAR_AUTO; c->graph_steps = -1;
     c->tile_rows = 0;

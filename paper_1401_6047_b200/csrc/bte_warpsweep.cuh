@@ -499,6 +499,16 @@ __global__ void __launch_bounds__(WarpCfg<S, K>::T, 1) warpsweep_kernel(const __
     asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
 
     // ---- active systems and this CTA's range of band-rows --------------------------------------------
+    // Static partition balanced by COST, not by rows: a segment costs its rows plus about 3 NS row-iterations of
+    // pipeline fill / drain and halo rows (slower, predicated iterations), so a range that spans a band boundary must
+    // get fewer rows.  Every band is charged c_over + rows cost units; the i-th boundary sits at cost i / gridDim.x
+    // of the total (boundaries that fall into a band's overhead snap to the band's first row).
+    auto range_cut = [&](const long long i, const long long nb) -> long long {
+        const long long c_over = 3 * Cfg::NS, band_cost = rows + c_over;
+        const long long y = (i * nb * band_cost) / gridDim.x;
+        const long long b = y / band_cost, r = y - b * band_cost;
+        return b * rows + min(max(r - c_over, 0LL), (long long)rows);
+    };
     long long n_active = L.n_batch;
     int a_first = 0;
     long long start, end;
@@ -522,10 +532,8 @@ __global__ void __launch_bounds__(WarpCfg<S, K>::T, 1) warpsweep_kernel(const __
             total += sh.scan[w];
         }
         n_active = total;
-        const long long units = n_active * upb;
-        const long long U = (units + gridDim.x - 1) / gridDim.x;
-        start = min((long long)blockIdx.x * U, units);
-        end = min(start + U, units);
+        start = range_cut(blockIdx.x, n_active * n_bands);
+        end = range_cut(blockIdx.x + 1, n_active * n_bands);
         if (start < end) {
             a_first = (int)(start / upb);
             const int a_last = (int)((end - 1) / upb);
@@ -538,10 +546,8 @@ __global__ void __launch_bounds__(WarpCfg<S, K>::T, 1) warpsweep_kernel(const __
             }
         }
     } else {
-        const long long units = n_active * upb;
-        const long long U = (units + gridDim.x - 1) / gridDim.x;
-        start = min((long long)blockIdx.x * U, units);
-        end = min(start + U, units);
+        start = range_cut(blockIdx.x, n_active * n_bands);
+        end = range_cut(blockIdx.x + 1, n_active * n_bands);
     }
     __syncthreads();   // mbarriers initialised, list visible, tensor memory allocated
     asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");

@@ -31,7 +31,7 @@ def test_default_workload_line():
     S = round(r["steps_per_launch"])
     assert d["steps"] == 60 and d["gpu_launches"] == 60 // S and S in (2, 3, 4)     # S time steps per launch
     assert r["bound"] == "hbm" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
-    assert r["kernel"] in ("sweep_kernel", "regsweep_kernel") and 0.3 < r["frac"] < 1.1
+    assert r["kernel"] in ("sweep_kernel", "warpsweep_kernel") and 0.3 < r["frac"] < 1.1
     assert r["one_step_per_pass"]["launches"] == r["one_step_per_pass"]["steps"]
     assert 0.5 < r["one_step_per_pass"]["frac"] < 1.1                         # the HBM-bound form of the kernel
     e = d["e2e"]

@@ -91,6 +91,19 @@ def test_streaming_configs_full_length_every_sweep_depth(idx, sweep_steps):
     run_and_compare(idx, variant=3, sweep_steps=sweep_steps)
 
 
+@pytest.mark.parametrize("idx", [3, 4])
+@pytest.mark.parametrize("sweep_steps", [2, 3])
+def test_streaming_configs_full_length_warp_kernel(idx, sweep_steps):
+    """The same through the warp kernel (variant 5: registers + tensor memory, bte_warpsweep.cuh); config 4 is what
+    the automatic choice runs."""
+    run_and_compare(idx, variant=5, sweep_steps=sweep_steps)
+
+
+def test_config2_full_length_warp_kernel():
+    """Config 2 (78 540 steps, 151 rows) through the warp kernel with graph replay."""
+    run_and_compare(2, variant=5)
+
+
 def test_config2_full_length_streaming_kernel():
     """Config 2 (78 540 steps) through the sweep kernel with graph replay instead of the resident kernel."""
     run_and_compare(2, variant=3)
