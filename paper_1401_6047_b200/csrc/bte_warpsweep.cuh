@@ -204,7 +204,7 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
     using Cfg = WarpCfg<S, K>;
     constexpr int NS = Cfg::NS, NV = Cfg::NV, HALO = Cfg::HALO, W = Cfg::W, REC = Cfg::REC;
     constexpr int DIN = Cfg::DIN, DPRE = Cfg::DPRE;
-    constexpr unsigned RB = REC * 16;                   // bytes per record
+    constexpr unsigned RB_BYTES = REC * 16;             // bytes per record
     const int lane = threadIdx.x & 31;
     const double2 zero = make_double2(0.0, 0.0);
 
@@ -271,7 +271,7 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
         // (the record that lived in this slot was read two iterations ago: those loads have long been consumed)
         if (rpre <= rho_end && elect_one()) {
             const unsigned slot = tpre & (DIN - 1);
-            const unsigned dst = ring + slot * RB, bar = bars + slot * 8;
+            const unsigned dst = ring + slot * RB_BYTES, bar = bars + slot * 8;
             mbar_arrive_expect_tx(bar, nA + nB);
             bulk_g2s(dst + dA, gA + min(max(rpre + 2, 0), rh_max) * pitch, nA, bar);
             bulk_g2s(dst + dB, gF + min(max(rpre + 1, 0), rf_max) * pitch, nB, bar);
@@ -298,43 +298,59 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
     const double* cnp = cn0 + (rho + 2);                // c_n of the row started by stage 0 (stage j: j rows back)
     unsigned tmS = tmP;                                 // tensor-memory address of stage 0's slot of this iteration
 
+    // take record r from the ring into registers (edge_tag: rows outside the lattice / the trapezoid read as zero)
+    double2 RA[K], RB[K], RFL, RFR;
+    // the answer of an mbarrier probe takes ~100 cycles: the probe for the next record is issued before the last
+    // stage of an iteration (`probe`), its answer is looked at when the record is taken
+    auto probe = [&]() { return mbar_try_wait(bars + (t_in & (DIN - 1)) * 8, (t_in / DIN) & 1u); };
+    auto take = [&](auto edge_tag, const int r, bool landed) {
+        constexpr bool EDGE = decltype(edge_tag)::value;
+        const unsigned slot = t_in & (DIN - 1);
+        while (!landed) landed = mbar_try_wait(bars + slot * 8, (t_in / DIN) & 1u);   // record r has landed
+        const unsigned src = a_lane + slot * RB_BYTES;
+        bool okh = true, okf = true;
+        if (EDGE) { okh = (unsigned)(r + 2) <= (unsigned)rh_max; okf = (unsigned)(r + 1) <= (unsigned)rf_max; }
+#pragma unroll
+        for (int q = 0; q < K; ++q) {
+            RA[q] = okh ? lds_d2_volatile(src + q * 16) : zero;
+            RB[q] = okf ? lds_d2_volatile(src + (Cfg::COLS + 1 + q) * 16) : zero;
+        }
+        RFL = okf ? lds_d2_volatile(src + Cfg::COLS * 16) : zero;
+        RFR = okf ? lds_d2_volatile(src + (Cfg::COLS + 1 + K) * 16) : zero;
+        ++t_in;
+    };
+    take(std::true_type{}, rho, false);
+
     // edge_tag: std::true_type = fill / drain iteration (row predicates, special rows 0 and 1)
     auto body = [&](auto edge_tag) {
         constexpr bool EDGE = decltype(edge_tag)::value;
 #ifndef BTE_NO_WAIT_ST
         tm_wait_st();                                   // the partial sums stored in the previous iterations are in place
 #endif
+        // E(t_v) dt/2 of the NV half-step times: broadcast reads, issued here so that the prefetch code below covers
+        // their latency (volatile: kept out of the loop-invariant registers)
+        double Ev[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) Ev[v] = *(volatile double*)(&tabp[v]);
         unsigned Praw[SL];
         tm_ld(tmS, Praw);                            // stage 0's rows in flight
-        // ---- take record rho ----
+        // ---- record rho: taken at the end of the previous iteration (its ring reads are hidden behind the loop edge) ----
         double2 Z[NS + 2][K];                           // Z[j + 2] = output of stage j; Z[0] = A, Z[1] = B
-        double2 FL, FR;                                 // F^0 columns left / right of this lane's K columns
-        {
-            prefetch();
-            const unsigned slot = t_in & (DIN - 1);
-            while (!mbar_try_wait(bars + slot * 8, (t_in / DIN) & 1u)) {}   // record rho has landed
-            const unsigned src = a_lane + slot * RB;
-            bool okh = true, okf = true;
-            if (EDGE) { okh = (unsigned)(rho + 2) <= (unsigned)rh_max; okf = (unsigned)(rho + 1) <= (unsigned)rf_max; }
 #pragma unroll
-            for (int q = 0; q < K; ++q) {
-                Z[0][q] = okh ? lds_d2_volatile(src + q * 16) : zero;
-                Z[1][q] = okf ? lds_d2_volatile(src + (Cfg::COLS + 1 + q) * 16) : zero;
-            }
-            FL = okf ? lds_d2_volatile(src + Cfg::COLS * 16) : zero;
-            FR = okf ? lds_d2_volatile(src + (Cfg::COLS + 1 + K) * 16) : zero;
-            ++t_in;
-        }
+        for (int q = 0; q < K; ++q) { Z[0][q] = RA[q]; Z[1][q] = RB[q]; }
+        const double2 FL = RFL, FR = RFR;               // F^0 columns left / right of this lane's K columns
+        prefetch();
         // mu[v][q] = n beta^{t_v}_m dt/2 of row n = rho - v + 2 (eq. 28-29): explicit mu of stage v, implicit mu' of stage v - 2
         double mu[NV][K];
         auto form_mu = [&](const int v) {
             const double ndv = nd0 + (double)(2 - v);
-            const double ndE = __dmul_rn(ndv, *(volatile double*)(&tabp[v]));
+            const double ndE = __dmul_rn(ndv, Ev[v]);
 #pragma unroll
             for (int q = 0; q < K; ++q) mu[v][q] = __fma_rn(ndv, bph[q], ndE);
         };
         // coefficients: they depend on (row, column, time) only, so the reciprocal chains are independent of each other
         // and of the data; they are formed for CG stages at a time (CG K independent chains side by side)
+        bool landed = false;
         form_mu(0);
         form_mu(1);
         double2 pq[NS][K];                              // (nu, mu') / (nu^2 + mu'^2) of stage j
@@ -355,6 +371,7 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
             const double2* ownp = Z[j];
             double2* Zo = Z[j + 2];
             const int n = rho - j;
+            if (j == NS - 1) landed = probe();
             bool comp = true, strt = true;
             if (EDGE) {
                 const int lo = max(0, lo_base + j), hi = min(N, hi_base - j);
@@ -429,10 +446,12 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
         ++rho; nd0 += 1.0;
         o_out += pitch; ++cnp;
         tmS ^= (unsigned)SL;                            // the other slot
+        if (EDGE) { if (rho <= rho_end) take(edge_tag, rho, landed); }
+        else take(edge_tag, rho, landed);               // steady state: the next record is a full one too
     };
 
     while (rho <= rho_end && rho < rho_s0) body(std::true_type{});
-    while (rho <= rho_s1) body(std::false_type{});
+    while (rho < rho_s1) body(std::false_type{});      // (the record taken at its end must be a steady one too)
     while (rho <= rho_end) body(std::true_type{});
 
     // per-strip partial sums of row 0 (a) and row 1 (b) of the S new whole grids -> eq. (12), (20)
