@@ -48,6 +48,9 @@
 #ifndef BTE_WS_DIN
 #define BTE_WS_DIN 8
 #endif
+#ifndef BTE_WS_COVER
+#define BTE_WS_COVER 6
+#endif
 #ifndef BTE_WS_CG
 #define BTE_WS_CG 3
 #endif
@@ -240,9 +243,12 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
     const int lo_base = r0 - HALO, hi_base = r0 + Lr - 1 + HALO;
     const int rho_start = max(0, lo_base) - 2;          // first / last iteration of the segment
     const int rho_end = min(N, r0 + Lr - 1) + NS - 1;
-    // steady state: every stage finishes a row >= 1 and starts a row of its range, stores in range, full records
-    const int rho_s0 = NS - 1 + max(r0, 1);
-    const int rho_s1 = min(N, hi_base) - 2;
+    // Unpredicated ("steady") iterations: every stage finishes a row >= 2 and starts a row <= N of the LATTICE, records are
+    // real rows.  The trapezoid of a segment that cuts a column in the middle needs no predicates: outside its range a
+    // stage forms values nobody uses (from real rows and finite partial sums), only the stores are limited to the
+    // segment's own rows.  Predicated iterations remain at the two ends of the lattice (rows 0, 1 and beyond N).
+    const int rho_s0 = max(rho_start, NS + 1);
+    const int rho_s1 = min(N - 2, rho_end);
 
     // ---- HBM -> input ring -------------------------------------------------------------------------------
     // record rho = (A = H^0 row rho + 2, columns c0 - HALO .. + COLS - 1;  B = F^0 row rho + 1, one column more on
@@ -407,7 +413,7 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
                     Zo[q] = cn_apply(Pq[q], D[q], kap[q], pq[j][q]);
                     if (EDGE && n == 0) Zo[q].y = 0.0;                // b_0 == 0 (eq. 23, C3)
                 }
-                const bool mine = !EDGE || (n >= r0 && n < r0 + Lr);
+                const bool mine = (n >= r0 && n < r0 + Lr);
                 if (j >= NS - 2 && mine) {                            // the two newest time levels go to HBM
                     double2* out = (j == NS - 1) ? Fout + (o_out - pitch) : Hout + o_out;
 #pragma unroll
@@ -523,7 +529,7 @@ __global__ void __launch_bounds__(WarpCfg<S, K>::T, 1) warpsweep_kernel(const __
     // get fewer rows.  Every band is charged c_over + rows cost units; the i-th boundary sits at cost i / gridDim.x
     // of the total (boundaries that fall into a band's overhead snap to the band's first row).
     auto range_cut = [&](const long long i, const long long nb) -> long long {
-        const long long c_over = 3 * Cfg::NS, band_cost = rows + c_over;
+        const long long c_over = BTE_WS_COVER * Cfg::NS / 2, band_cost = rows + c_over;
         const long long y = (i * nb * band_cost) / gridDim.x;
         const long long b = y / band_cost, r = y - b * band_cost;
         return b * rows + min(max(r - c_over, 0LL), (long long)rows);
