@@ -233,7 +233,7 @@ SweepFn sweep_fn(int S, bool budgets, int wide) {
     }
 }
 constexpr int RING_MAX_STEPS = 3;   // the shared-memory-ring kernel is instantiated for S = 1 .. 3
-constexpr int WARP_MIN_ROWS = 96;   // automatic choice of the warp kernel: columns at least this long (measured: config 3, 41 rows, is faster on the ring kernel)
+constexpr int WARP_MIN_ROWS = 32;   // automatic choice of the warp kernel: columns at least this long (config 3, 41 rows: 126 G against 105 G on the ring kernel)
 constexpr int WS_MAX_STEPS = 3;     // the register-resident kernel is instantiated for S = 2, 3
 static_assert(WS_MAX_STEPS <= SWEEP_MAX_STEPS, "partial sums are laid out for SWEEP_MAX_STEPS steps per pass");
 
@@ -280,8 +280,8 @@ int plan_sweep(bte_ctx* c) {
                         cudaGetErrorString(e));
         if (occ < 1) continue;
         const long long strips = (c->grid.n_phiy + f.W - 1) / f.W;
-        const long long bands = (strips + f.strips_per_band - 1) / f.strips_per_band;
-        const long long units = bands * (c->grid.n_harm + 1) * (long long)c->grid.n_batch;
+        const long long bands = (strips * c->grid.n_batch + f.strips_per_band - 1) / f.strips_per_band;
+        const long long units = bands * (c->grid.n_harm + 1);
         if (2LL * c->grid.n_batch * rows_alloc * c->off.pitch >= (1LL << 31)) continue;   // 32-bit element offsets
         if (strips * (c->grid.n_harm + 1) >= (1LL << 31) || units >= (1LL << 31)) continue;
         long long g = (long long)sms * occ;

@@ -29,9 +29,10 @@
 //   the NS x 2 x K partial right-hand sides.  mu of row n at time t_v is the implicit mu' of stage v - 2 and the
 //   explicit mu of stage v in the same iteration: formed once.
 //
-// Work decomposition: bands of WARPS adjacent strips; band-rows (system, band, n) are numbered consecutively and
-// dealt out in equal contiguous ranges to one CTA per SM; warp g of the CTA takes strip g of the band, so the warps
-// of a CTA touch adjacent 1 KB runs of every row (DRAM page locality).
+// Work decomposition: the (active system, strip) pairs are numbered consecutively and grouped into bands of WARPS; the
+// band-rows (band, n) are dealt out in contiguous ranges of equal COST to one CTA per SM; warp g of the CTA takes pair g
+// of the band, so the warps of a CTA touch adjacent 1.5 KB runs of every row (DRAM page locality), and a batch of narrow
+// systems fills every warp.
 // Per-step reductions (eq. 12, 17, 20): the even stages see rows 0 and 1 of the new whole grids -> per-strip partial
 // sums -> fixed-order fold by the warp that completes a system (fold_sweep, bte_sweep.cuh).
 #pragma once
@@ -505,9 +506,9 @@ __global__ void __launch_bounds__(WarpCfg<S, K>::T, 1) warpsweep_kernel(const __
     const int warp = uni(i >> 5);
     const int rows = L.N + 1;
     const int n_strips = (L.M1 + W - 1) / W;
-    const int n_bands = (n_strips + WARPS - 1) / WARPS;
     const unsigned ups = (unsigned)n_strips * (unsigned)rows;                 // row-units per system
-    const long long upb = (long long)n_bands * rows;                          // band-rows per system
+    // bands of WARPS consecutive (active system, strip) pairs: a band may straddle two systems of a batch
+    auto bands_of = [&](const long long n_act) -> long long { return (n_act * n_strips + WARPS - 1) / WARPS; };
 
     const unsigned base = (unsigned)__cvta_generic_to_shared(ws_smem) + (unsigned)warp * (unsigned)Cfg::warp_bytes;
     const unsigned ring = base, bars = base + (unsigned)Cfg::off_bars;
@@ -557,11 +558,11 @@ __global__ void __launch_bounds__(WarpCfg<S, K>::T, 1) warpsweep_kernel(const __
             total += sh.scan[w];
         }
         n_active = total;
-        start = range_cut(blockIdx.x, n_active * n_bands);
-        end = range_cut(blockIdx.x + 1, n_active * n_bands);
+        start = range_cut(blockIdx.x, bands_of(n_active));
+        end = range_cut(blockIdx.x + 1, bands_of(n_active));
         if (start < end) {
-            a_first = (int)(start / upb);
-            const int a_last = (int)((end - 1) / upb);
+            a_first = (int)((start / rows) * WARPS / n_strips);
+            const int a_last = (int)min(n_active - 1, (((end - 1) / rows) * WARPS + WARPS - 1) / n_strips);
             int a = base_a + incl - cnt;                  // index of this thread's first active system
             for (int s = s_lo; s < s_hi; ++s) {
                 if (sys_active(L, s, S)) {
@@ -571,8 +572,8 @@ __global__ void __launch_bounds__(WarpCfg<S, K>::T, 1) warpsweep_kernel(const __
             }
         }
     } else {
-        start = range_cut(blockIdx.x, n_active * n_bands);
-        end = range_cut(blockIdx.x + 1, n_active * n_bands);
+        start = range_cut(blockIdx.x, bands_of(n_active));
+        end = range_cut(blockIdx.x + 1, bands_of(n_active));
     }
     __syncthreads();   // mbarriers initialised, list visible, tensor memory allocated
     asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
@@ -581,15 +582,17 @@ __global__ void __launch_bounds__(WarpCfg<S, K>::T, 1) warpsweep_kernel(const __
     // ---- every warp walks the CTA's range segment by segment: its strip of the band ----------------------
     long long pos = start;
     while (pos < end) {
-        const int a = (int)(pos / upb);
-        const int rem = (int)(pos - (long long)a * upb);
-        const int band = rem / rows;
-        const int r0 = rem - band * rows;
+        const long long band = pos / rows;
+        const int r0 = (int)(pos - band * rows);
         const int Lr = (int)min((long long)(rows - r0), end - pos);
-        const int sys = BUDGETS ? uni(sh.list[a - a_first]) : a;
-        const int strip = band * WARPS + warp;
+        const long long g = band * WARPS + warp;          // this warp's (active system, strip) pair
         pos += Lr;
-        if (strip < n_strips) warpsweep_segment<S, K>(L, sys, strip, r0, Lr, n_strips, ups, ring, tabp, bars, tmP, accs, t_in);
+        if (g < n_active * n_strips) {
+            const int a = (int)(g / n_strips);
+            const int strip = (int)(g - (long long)a * n_strips);
+            const int sys = BUDGETS ? uni(sh.list[a - a_first]) : a;
+            warpsweep_segment<S, K>(L, sys, strip, r0, Lr, n_strips, ups, ring, tabp, bars, tmP, accs, t_in);
+        }
     }
 
     // ---- the last CTA of the launch advances the step counters of all systems that were active --------
