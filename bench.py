@@ -303,6 +303,8 @@ def apply_options(s, args, sweep_steps=None, variant=None):
         s.set_option("sweep_ctas", args.ctas)
     if args.res_ctas:
         s.set_option("resident_ctas", args.res_ctas)
+    if args.res_halo:
+        s.set_option("resident_halo", args.res_halo)
     if args.sweep_threads:
         s.set_option("sweep_threads", args.sweep_threads)
 
@@ -546,6 +548,7 @@ def main():
                          "reported with dtype f32 -- not the BASELINE metric)")
     ap.add_argument("--sweep-threads", type=int, default=0, help="threads per CTA of the sweep kernel (0 auto)")
     ap.add_argument("--res-ctas", type=int, default=0, help="slabs of the resident kernel (0 auto)")
+    ap.add_argument("--res-halo", type=int, default=0, help="halo columns of the resident kernel's grid mode (0 auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true", help="time the headline workload only")
     ap.add_argument("--ref-budget", type=float, default=2.5e9,

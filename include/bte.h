@@ -200,7 +200,9 @@ BTE_API int bte_rs_destroy(bte_rs_ctx* ctx);
  *                      choice: 4 when usable, n_steps >= 4 and (for a batch) systems of at most 8192 points.
  *   "resident_ctas" slabs (CTAs) of variant 4: 1 = one CTA, 2..16 = one thread-block cluster, more = cooperative
  *                  grid; 0 = automatic
- *   "sweep_steps"  S of variant 3 (1..3) or 5 (2..4), 0 = automatic
+ *   "resident_halo" halo columns per side of a slab in the cooperative-grid mode of variant 4 (1..4): neighbours
+ *                  exchange their edge columns once per that many half-updates; 0 = automatic (3)
+ *   "sweep_steps"  S of variant 3 (1..3) or 5 (2..3), 0 = automatic
  *   "sweep_ctas"   CTAs of the persistent sweep kernel, 0 = SMs x resident CTAs
  *   "sweep_threads" threads per CTA of the sweep kernel: 128, 256 or (one-step pass only) 512, 0 = automatic
  *   "graph_steps"  launches captured per CUDA graph for launch-bound grids; 0 = plain launches, -1 = auto

@@ -104,7 +104,7 @@ Offsets offsets_for(const bte_grid* g) {
     // resident variant: edge columns of both grids of every slab, per-slab sums
     o.rhalo = off;
     if (resident_possible(g) && g->n_batch == 1)
-        off = align_up(off + (size_t)2 * RES_MAX_CTAS * 2 * (g->n_harm + 1) * sizeof(double2));
+        off = align_up(off + (size_t)2 * RES_MAX_HALO * 2 * RES_MAX_CTAS * 2 * (g->n_harm + 1) * sizeof(double2));
     o.rout = off;    off = align_up(off + std::max<size_t>(RES_MAX_CTAS, (size_t)g->n_batch * 16) * 8 * sizeof(double));
     o.rflag = off;   off = align_up(off + (size_t)RES_MAX_CTAS * sizeof(unsigned int));
     o.total = off;
@@ -161,7 +161,8 @@ struct bte_ctx {
     // resident (on-chip) kernel launch plan
     int res_ctas_opt;                // option: slabs (0 = automatic)
     int res_mode;                    // -1 = not usable; 0 one CTA, 1 one cluster, 2 cooperative grid
-    int res_G, res_Wc, res_T;
+    int res_G, res_Wc, res_T, res_HB;
+    int res_halo_opt;                // option: halo columns of the grid mode (0 = automatic)
     size_t res_smem;
     // CUDA graph cache
     cudaGraph_t graph;
@@ -342,10 +343,18 @@ bool resident_try(bte_ctx* c, int mode, int G) {
     const int Ge = (M1 + wc - 1) / wc;          // slabs actually needed with this width
     if ((mode == 0) != (Ge == 1)) return false;
     if (mode == 1 && Ge != G) return false;    // cluster sizes are taken as given (2, 4, 8, 16)
-    const size_t smem = resident_smem_bytes(N, wc);
+    // grid mode: HB halo columns per side, one neighbour exchange per HB half-updates (bte_resident.cuh); every slab,
+    // the last one included, must own at least HB columns
+    int hb = 1;
+    if (mode == 2) {
+        hb = c->res_halo_opt > 0 ? c->res_halo_opt : 3;
+        const int last = M1 - (Ge - 1) * wc;
+        while (hb > 1 && (last < hb || resident_smem_bytes(N, wc, hb) > RES_SMEM_CAP)) --hb;
+    }
+    const size_t smem = resident_smem_bytes(N, wc, hb);
     if (smem > RES_SMEM_CAP) return false;
     void* fn = resident_fn(mode);
-    const int T = resident_threads(N + 1, wc);
+    const int T = resident_threads(N + 1, wc + 2 * (hb - 1));
     if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
         cudaGetLastError();
         return false;
@@ -376,7 +385,7 @@ bool resident_try(bte_ctx* c, int mode, int G) {
             return false;
         }
     }
-    c->res_mode = mode; c->res_G = Ge; c->res_Wc = wc; c->res_T = T; c->res_smem = smem;
+    c->res_mode = mode; c->res_G = Ge; c->res_Wc = wc; c->res_T = T; c->res_smem = smem; c->res_HB = hb;
     return true;
 }
 
@@ -408,7 +417,7 @@ int plan_resident(bte_ctx* c) {
 
 int launch_resident(bte_ctx* c, int64_t n_steps) {
     ResidentArgs A{};
-    A.G = c->res_G; A.Wc = c->res_Wc; A.T = c->res_T; A.n_steps = n_steps;
+    A.G = c->res_G; A.Wc = c->res_Wc; A.T = c->res_T; A.n_steps = n_steps; A.HB = c->res_HB;
     A.halo = (double2*)(c->ws + c->off.rhalo);
     A.cta_out = (double*)(c->ws + c->off.rout);
     A.flag = (unsigned int*)(c->ws + c->off.rflag);
@@ -723,6 +732,7 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
     c->budgets.erase(std::unique(c->budgets.begin(), c->budgets.end()), c->budgets.end());
     c->sweep_steps = 0; c->sweep_ctas = 0; c->sm_count = 0; c->graph_S = 0; c->sweep_threads = 0;
     c->res_ctas_opt = 0; c->res_mode = -1; c->res_G = 0; c->res_Wc = 0; c->res_T = 0; c->res_smem = 0;
+    c->res_HB = 1; c->res_halo_opt = 0;
     for (int S = 0; S <= SWEEP_MAX_STEPS; ++S) c->sw_grid[S] = c->ws_grid[S] = 0;
     c->steps_issued = 0; c->launches = 0;
     c->variant = VAR_AUTO; c->graph_steps = -1;
@@ -1087,6 +1097,11 @@ int bte_set_option(bte_ctx* c, const char* key, int64_t value) {
     if (!strcmp(key, "resident_ctas")) {   // slabs of the resident kernel: 1 = one CTA, 2..16 = cluster, more = grid
         if (value < 0 || value > RES_MAX_CTAS) return fail(BTE_EINVAL, "resident_ctas must be in [0, %d]", RES_MAX_CTAS);
         c->res_ctas_opt = (int)value;
+        return plan_resident(c);
+    }
+    if (!strcmp(key, "resident_halo")) {   // halo columns per side of the resident kernel's grid mode (0 = automatic)
+        if (value < 0 || value > RES_MAX_HALO) return fail(BTE_EINVAL, "resident_halo must be in [0, %d]", RES_MAX_HALO);
+        c->res_halo_opt = (int)value;
         return plan_resident(c);
     }
     if (!strcmp(key, "sweep_threads")) {   // threads per CTA of the sweep kernel: 128 or 256 (0 = automatic)

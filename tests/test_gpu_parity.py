@@ -141,6 +141,23 @@ def test_resident_slabs(res_ctas):
     s.destroy()
 
 
+@pytest.mark.parametrize("halo", [1, 2, 3, 4])
+@pytest.mark.parametrize("res_ctas", [17, 37, 75])
+def test_resident_grid_halo_width(res_ctas, halo):
+    """Cooperative-grid mode with 1..4 halo columns per side: the slabs exchange edge columns once per `halo`
+    half-updates and update the halo columns redundantly in between (trapezoid in time); odd and even step counts,
+    launches that end in the middle of an exchange group."""
+    w = W.small_case(N=21, M1=300, dt=0.004, n_steps=23, avg_start=3)
+    s = gpu_solver(w, "resident", res_ctas=res_ctas)
+    s.set_option("resident_halo", halo)
+    s.step(5); s.step(1); s.step(10); s.step(7)
+    obs = s.observables()
+    sim = oracle_run(w, 23)[0]
+    assert_state_close(s, sim, 0, what=f"resident grid ctas={res_ctas} halo={halo}")
+    assert_obs_close(obs[0], sim.observables(), w.params[0], w.grid.dt, what=f"resident grid ctas={res_ctas} halo={halo}")
+    s.destroy()
+
+
 @pytest.mark.parametrize("res_ctas", [1, 2, 4, 0])
 def test_resident_batched_with_budgets(res_ctas):
     """A batch on the resident kernel: one CTA / one cluster per system, every system ends at its own step budget;
