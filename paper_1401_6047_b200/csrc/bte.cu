@@ -406,6 +406,18 @@ int plan_resident(bte_ctx* c) {
     // CTAs); synchronisation cost grows with the number of CTAs: __syncthreads < cluster barrier < neighbour
     // flags through L2
     if (pts <= 512 && resident_try(c, 0, 1)) return BTE_OK;
+    // one system of more than 16 x 512 points: cooperative grid with 3 halo columns per side (one neighbour exchange per
+    // 3 half-updates), as many slabs as leave about one point per thread and half-update (measured: config 1 5.5 us per
+    // step on a cluster of 16, 3.5 us on a grid of 67; config 2 9.0 -> 7.1 us on 148 slabs)
+    if (c->grid.n_batch == 1 && pts > 16 * 512) {
+        const int hb = c->res_halo_opt > 0 ? c->res_halo_opt : 3;
+        const int rows = c->grid.n_harm + 1;
+        int own = 992 / rows - 2 * (hb - 1);
+        if (own < hb) own = hb;
+        int G = (c->grid.n_phiy + own - 1) / own;
+        if (G > maxg) G = maxg;
+        if (G > 16 && resident_try(c, 2, G)) return BTE_OK;
+    }
     for (int G = 2; G <= 16; G *= 2)
         if ((pts / G <= 512 || G == 16) && resident_try(c, 1, G)) return BTE_OK;
     for (int G = 8; G >= 2; G /= 2)             // 16 not schedulable / does not fit: smaller clusters that fit

@@ -27,7 +27,13 @@
 #pragma once
 #include "bte_kernels.cuh"
 
+#ifndef BTE_RES_UNROLL
+#define BTE_RES_UNROLL 1
+#endif
+
 namespace bte {
+
+constexpr int RES_UNROLL = BTE_RES_UNROLL;   // rows of the column march per loop trip
 
 struct ResidentArgs {
     int G;                 // slabs = CTAs
@@ -134,6 +140,7 @@ __device__ __forceinline__ void resident_column(unsigned sX, unsigned sS, int nA
     double2 d1 = diff(a + PB);                                  // row n
     unsigned cna = scn + (unsigned)nA * 8;
     double nd = (double)nA;
+#pragma unroll RES_UNROLL
     for (int n = nA; n < nB; ++n) {
         a += PB;                                                // row n
         const double2 d2 = diff(a + PB);                        // row n + 1
