@@ -339,12 +339,14 @@ def timed_blocks(cx, s, w, steps, k_done, min_blocks, sample_clocks, max_blocks=
     return statistics.median(times), times, launches, k_done
 
 
-def hbm_roofline(w, updates_per_block, ms, launches, steps, variant, S, peak, peak_src):
+def hbm_roofline(w, updates_per_block, ms, launches, steps, variant, S, peak, peak_src, precision=0):
     """One launch of a sweep kernel advances every active system by S time steps in one pass over the state
     (temporal blocking): what that launch must move is the state read once and written once = 64 B per lattice
     point PER LAUNCH; the other variants move 96 / 64 B per point per step."""
     per_launch_s = ms * 1e-3 / max(1, launches)
     alg_bytes = VARIANT_BYTES[variant] * updates_per_block / steps       # per launch (sweep) / per step (others)
+    if precision != 0:
+        alg_bytes *= 0.5                                                  # fp32 pairs in HBM
     if variant in (3, 5):
         achieved = alg_bytes / per_launch_s / 1e9
     else:
@@ -392,14 +394,14 @@ def time_workload(cx, w, steps, warmup, min_blocks, sample_clocks, one_pass=Fals
     updates = w.updates_between(warm, warm + steps)
     last_updates = w.updates_between(k_done - steps, k_done)
     obs = s.observables()[0]
-    variant = s.get_option("effective_variant") if args.precision == 0 else 1
+    variant = s.get_option("effective_variant") if args.precision != 2 else 1
     S = s.get_option("effective_sweep_steps") if variant in (3, 5) else 1
     resident = launches == 1 and steps > 1 and args.precision == 0
     out = {"value": updates * cx.world / (ms * 1e-3), "ms_per_step": ms / steps, "steps": steps,
            "blocks": len(times), "ms_min_max": [min(times) / steps, max(times) / steps],
            "gpu_launches": launches, "same_work_every_block": updates == last_updates,
            "roofline": (alu_roofline(updates, ms, steps, launches) if resident else
-                        hbm_roofline(w, updates, ms, launches, steps, variant, S, peak, peak_src)),
+                        hbm_roofline(w, updates, ms, launches, steps, variant, S, peak, peak_src, args.precision)),
            "check": {"norm": obs.norm, "v_dr": obs.v_dr, "step": obs.step}}
     out["kernel"] = out["roofline"]["kernel"]
     # The same workload with ONE time step per pass (sweep_steps = 1): the plain HBM-bound form of the step

@@ -69,9 +69,10 @@ typedef struct {
     int32_t n_harm;  /* N  : highest harmonic kept, rows n = 0..N            [n-harmonics]               */
     int32_t n_phiy;  /* M+1: number of phi_y lattice points, m = 0..M        [g-grid]                    */
     int32_t n_batch; /* number of independent systems advanced together, >= 1                            */
-    int32_t precision;/* 0 = fp64 (default; every kernel).  fp32 variants of the step (the paper's precision, L311;
-                        two launches per step, streaming / resident kernels not used): 1 = state stored as fp32,
-                        arithmetic fp64; 2 = fp32 storage and arithmetic.  Host arrays stay double.          */
+    int32_t precision;/* 0 = fp64 (default; every kernel).  fp32 variants of the step (the paper's precision, L311):
+                        1 = state stored as fp32 pairs, arithmetic fp64 (multi-step passes through the warp kernel
+                        on lattices of >= 32 rows, otherwise two launches per step); 2 = fp32 storage and arithmetic
+                        (two launches per step).  The resident kernel is fp64 only.  Host arrays stay double.   */
     double dt;       /* time step in units of tau                            [dt]                        */
 } bte_grid;
 

@@ -240,17 +240,16 @@ static_assert(WS_MAX_STEPS <= SWEEP_MAX_STEPS, "partial sums are laid out for SW
 
 // register-resident warp kernel (bte_warpsweep.cuh): S = 2, 3 steps per pass, K = BTE_WS_K columns per lane
 constexpr int WS_K = BTE_WS_K;
-template <int S>
+// EB = bytes of a stored pair: 16 (fp64 state) or 8 (bte_grid.precision 1: fp32 storage, fp64 arithmetic)
+template <int S, int EB>
 SweepFn warpsweep_fn_s(bool budgets) {
-    using Cfg = WarpCfg<S, WS_K>;
-    return {budgets ? (void*)warpsweep_kernel<S, WS_K, true> : (void*)warpsweep_kernel<S, WS_K, false>,
+    using Cfg = WarpCfg<S, WS_K, EB>;
+    return {budgets ? (void*)warpsweep_kernel<S, WS_K, true, EB> : (void*)warpsweep_kernel<S, WS_K, false, EB>,
             Cfg::smem_bytes, Cfg::W, Cfg::T, Cfg::WARPS};
 }
-SweepFn warpsweep_fn(int S, bool budgets) {
-    switch (S) {
-        case 2: return warpsweep_fn_s<2>(budgets);
-        default: return warpsweep_fn_s<3>(budgets);
-    }
+SweepFn warpsweep_fn(int S, bool budgets, int precision) {
+    if (precision == 1) return S == 2 ? warpsweep_fn_s<2, 8>(budgets) : warpsweep_fn_s<3, 8>(budgets);
+    return S == 2 ? warpsweep_fn_s<2, 16>(budgets) : warpsweep_fn_s<3, 16>(budgets);
 }
 
 // Wider CTAs pay off only for the HBM-bound one-step pass over long rows (4 or 8 KB DRAM bursts per row instead
@@ -264,7 +263,7 @@ int sweep_wide(const bte_ctx* c, int S) {
 
 int plan_sweep(bte_ctx* c) {
     for (int S = 0; S <= SWEEP_MAX_STEPS; ++S) c->sw_grid[S] = c->ws_grid[S] = 0;
-    if (c->grid.precision != 0) return BTE_OK;     // fp32 variants run the split kernels only
+    if (c->grid.precision == 2) return BTE_OK;     // fp32 arithmetic: the split kernels only
     int dev = 0, sms = 0;
     CUDA_TRY(cudaGetDevice(&dev));
     CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -272,7 +271,7 @@ int plan_sweep(bte_ctx* c) {
     const long long rows_alloc = c->grid.n_harm + 1 + 2 * GHOST;
     // warp kernel: one CTA of WARPS independent warps per SM; a CTA range is counted in band-rows
     for (int S = 2; S <= WS_MAX_STEPS; ++S) {
-        const SweepFn f = warpsweep_fn(S, c->has_budgets);
+        const SweepFn f = warpsweep_fn(S, c->has_budgets, c->grid.precision);
         int occ = 0;
         cudaError_t e = cudaFuncSetAttribute(f.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)f.smem);
         if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, f.fn, f.T, f.smem);
@@ -294,7 +293,7 @@ int plan_sweep(bte_ctx* c) {
         if (c->has_budgets && (long long)c->grid.n_batch / g + 2 > WarpCfg<2, WS_K>::MAX_SPAN) continue;
         c->ws_grid[S] = (int)g;
     }
-    for (int S = 1; S <= RING_MAX_STEPS; ++S) {
+    for (int S = 1; S <= RING_MAX_STEPS && c->grid.precision == 0; ++S) {
         c->sw_grid[S] = 0;
         const SweepFn f = sweep_fn(S, c->has_budgets, sweep_wide(c, S));
         int occ = 0;
@@ -457,7 +456,14 @@ int launch_resident(bte_ctx* c, int64_t n_steps) {
 }
 
 int effective_variant(const bte_ctx* c) {
-    if (c->grid.precision != 0) return VAR_SPLIT;
+    if (c->grid.precision == 2) return VAR_SPLIT;
+    if (c->grid.precision == 1) {
+        // fp32 storage: multi-step passes through the warp kernel (half the HBM bytes), single steps (remainders, budget
+        // cuts) through the two-launch form
+        const bool ok = c->ws_grid[WS_MAX_STEPS] > 0 && c->grid.n_harm + 1 >= WARP_MIN_ROWS;
+        return ok && (c->variant == VAR_AUTO || c->variant == VAR_WARPSWEEP || c->variant == VAR_RESIDENT) ? VAR_WARPSWEEP
+                                                                                                         : VAR_SPLIT;
+    }
     // one-step launches of the warp kernel's plan run the ring kernel (the HBM-bound form), so both must be usable
     const bool warp_ok = c->sw_grid[1] > 0 && c->ws_grid[2] > 0;
     if (c->variant == VAR_WARPSWEEP && warp_ok) return VAR_WARPSWEEP;
@@ -475,7 +481,7 @@ bool is_sweep(int var) { return var == VAR_SWEEP || var == VAR_WARPSWEEP; }
 // is an s-step launch available in the effective streaming variant?  (one-step launches always run the
 // shared-memory-ring kernel: the HBM-bound form, bte_sweep.cuh)
 bool sweep_has(const bte_ctx* c, int var, int s) {
-    if (s == 1) return c->sw_grid[1] > 0;
+    if (s == 1) return c->grid.precision == 0 ? c->sw_grid[1] > 0 : true;   // fp32 storage: the two-launch form
     return var == VAR_WARPSWEEP ? c->ws_grid[s] > 0 : (s <= RING_MAX_STEPS && c->sw_grid[s] > 0);
 }
 
@@ -499,7 +505,7 @@ int sweep_steps(const bte_ctx* c) {
 SweepFn sweep_launch(const bte_ctx* c, int var, int s, int* grid) {
     if (var == VAR_WARPSWEEP && s >= 2) {
         *grid = c->ws_grid[s];
-        return warpsweep_fn(s, c->has_budgets);
+        return warpsweep_fn(s, c->has_budgets, c->grid.precision);
     }
     *grid = c->sw_grid[s];
     return sweep_fn(s, c->has_budgets, sweep_wide(c, s));
@@ -530,7 +536,8 @@ int launches_per_step(const bte_ctx* c) { return effective_variant(c) == VAR_SPL
 // Issue one launch group with plain launches: S steps (sweep kernel) or one step (other variants).
 int launch_steps(bte_ctx* c, int S) {
     const int var = effective_variant(c);
-    if (is_sweep(var)) {
+    const bool single32 = c->grid.precision != 0 && S == 1;   // fp32 storage: single steps in the two-launch form
+    if (is_sweep(var) && !single32) {
         int grid = 0;
         const SweepFn f = sweep_launch(c, var, S, &grid);
         void* args[] = {&c->L};
@@ -554,7 +561,7 @@ int launch_steps(bte_ctx* c, int S) {
         }
     }
     CUDA_TRY(cudaGetLastError());
-    c->launches += launches_per_step(c);
+    c->launches += single32 ? 3 : launches_per_step(c);
     return BTE_OK;
 }
 

@@ -58,7 +58,8 @@
 
 namespace bte {
 
-template <int S, int K>
+// EB: bytes of one stored (a, b) pair: 16 (fp64 state) or 8 (fp32 storage, bte_grid.precision 1; arithmetic stays fp64)
+template <int S, int K, int EB = 16>
 struct WarpCfg {
     static constexpr int NS = 2 * S;            // half-updates (stages) per pass
     static constexpr int NV = NS + 2;           // half-step times of a pass
@@ -69,7 +70,9 @@ struct WarpCfg {
     static constexpr int T = 32 * WARPS;
     static constexpr int DIN = BTE_WS_DIN;      // slots of the HBM input ring
     static constexpr int DPRE = DIN - 2;              // rows prefetched ahead (the slot of record t + DPRE was read 2 iterations ago)
-    static constexpr int REC = 2 * COLS + 2;    // double2 per record: A = COLS columns, B = COLS + 2 columns, natural order
+    static constexpr int AX = EB == 8 ? 1 : 0;  // fp32 pairs: the A part starts one column early (16-byte alignment of the copies)
+    static constexpr int ACOLS = COLS + 2 * AX; // columns of the A part of a record
+    static constexpr int REC = ACOLS + COLS + 2; // pairs per record: A = ACOLS columns, B = COLS + 2 columns, natural order
     static constexpr int CG = BTE_WS_CG < 2 * S ? BTE_WS_CG : 2 * S;   // stages whose coefficients are formed together
     static constexpr int MAX_SPAN = 64;         // distinct systems one CTA range may touch
     // tensor memory: warp w owns the 32 lanes of quadrant w % 4, columns (w / 4) * TM_COLS .. + 2 NS TM_SLOT - 1;
@@ -80,7 +83,7 @@ struct WarpCfg {
     static constexpr int TM_ALLOC = TM_NEED <= 32 ? 32 : TM_NEED <= 64 ? 64 : TM_NEED <= 128 ? 128 : TM_NEED <= 256 ? 256 : 512;
     static_assert(4 * K <= TM_SLOT && TM_NEED <= 512, "tensor memory budget");
     // shared memory of one warp: input ring | E(t_v) dt/2 at the NV half-step times | mbarriers | reduction slots [S][2][32]
-    static constexpr size_t off_tab = (size_t)DIN * REC * 16;
+    static constexpr size_t off_tab = (size_t)DIN * REC * EB;
     static constexpr size_t off_bars = off_tab + (size_t)NV * 8;
     static constexpr size_t off_accs = off_bars + (size_t)DIN * 8;
     static constexpr size_t warp_bytes = off_accs + (size_t)S * 2 * 32 * 8;
@@ -117,6 +120,21 @@ __device__ __forceinline__ double2 lds_d2_volatile(unsigned addr) {
 __device__ __forceinline__ void sts_d2_volatile(unsigned addr, double2 v) {
     asm volatile("st.volatile.shared.v2.f64 [%0], {%1, %2};\n" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory");
 }
+// one stored pair from the ring -> fp64 (fp32 storage: widened, exact)
+template <int EB>
+__device__ __forceinline__ double2 lds_pair(unsigned addr) {
+    if constexpr (EB == 16) {
+        return lds_d2_volatile(addr);
+    } else {
+        float2 v;
+        asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [%2];\n" : "=f"(v.x), "=f"(v.y) : "r"(addr) : "memory");
+        return make_double2((double)v.x, (double)v.y);
+    }
+}
+template <int EB> struct PairOf { using type = double2; };
+template <> struct PairOf<8> { using type = float2; };
+__device__ __forceinline__ void st_pair(double2* p, double2 v) { *p = v; }
+__device__ __forceinline__ void st_pair(float2* p, double2 v) { *p = make_float2((float)v.x, (float)v.y); }   // rounded once
 // ---- 1-D bulk copies (TMA engine, SASS UBLKCP) with mbarrier completion: the HBM input ring ----
 __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
@@ -200,15 +218,16 @@ __device__ __forceinline__ unsigned uni(unsigned v) { return __shfl_sync(0xfffff
 //   ring, bars: shared addresses of this warp's input ring and mbarriers; tabp: its table of E(t_v) dt/2; accs: its
 //   reduction slots;
 //   t_in: records taken so far in this launch (slot and mbarrier phase of the next one).
-template <int S, int K>
+template <int S, int K, int EB>
 __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys, const int strip, const int r0,
                                                   const int Lr, const int n_strips, const unsigned ups,
                                                   const unsigned ring, double* tabp, const unsigned bars,
                                                   const unsigned tmP, double* __restrict__ accs, unsigned& t_in) {
-    using Cfg = WarpCfg<S, K>;
-    constexpr int NS = Cfg::NS, NV = Cfg::NV, HALO = Cfg::HALO, W = Cfg::W, REC = Cfg::REC;
+    using Cfg = WarpCfg<S, K, EB>;
+    using ST = typename PairOf<EB>::type;            // stored pair
+    constexpr int NS = Cfg::NS, NV = Cfg::NV, HALO = Cfg::HALO, W = Cfg::W, REC = Cfg::REC, AX = Cfg::AX;
     constexpr int DIN = Cfg::DIN, DPRE = Cfg::DPRE;
-    constexpr unsigned RB_BYTES = REC * 16;             // bytes per record
+    constexpr unsigned RB_BYTES = REC * EB;             // bytes per record
     const int lane = threadIdx.x & 31;
     const double2 zero = make_double2(0.0, 0.0);
 
@@ -256,24 +275,25 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
     // each side), natural column order.  Columns outside [0, pitch) are not copied: those parts of the ring are
     // zeroed once per segment (boundary condition (22)-(23) in m; the pad columns M+1 .. pitch-1 are zero in HBM).
     // Rows outside the lattice / the segment's trapezoid are not copied either: the record reads as zero.
-    const double2* __restrict__ Hin = state_ptr(L, cur, 0, sys);   // row 0, column 0
+    const ST* __restrict__ Hin = (const ST*)L.state + (((size_t)cur * 2) * L.n_batch + sys) * grid_points(L) +
+                                 (size_t)GHOST * pitch;   // whole grid of the live buffer: row 0, column 0
     const int rf_max = min(N, hi_base + 1), rh_max = min(N, hi_base);      // last F^0 / H^0 row needed
-    const int wa = c0 - HALO, wb = wa - 1;              // first column of the A / B part of a record
-    const int ca0 = max(0, wa), ca1 = min(pitch, wa + Cfg::COLS);
+    const int wa = c0 - HALO - AX, wb = c0 - HALO - 1;  // first column of the A / B part of a record
+    const int ca0 = max(0, wa), ca1 = min(pitch, wa + Cfg::ACOLS);
     const int cb0 = max(0, wb), cb1 = min(pitch, wb + Cfg::COLS + 2);
-    const unsigned nA = (unsigned)(ca1 - ca0) * 16u, nB = (unsigned)(cb1 - cb0) * 16u;
-    const unsigned dA = (unsigned)(ca0 - wa) * 16u, dB = (unsigned)(Cfg::COLS + cb0 - wb) * 16u;   // offsets in a record
+    const unsigned nA = (unsigned)(ca1 - ca0) * EB, nB = (unsigned)(cb1 - cb0) * EB;
+    const unsigned dA = (unsigned)(ca0 - wa) * EB, dB = (unsigned)(Cfg::ACOLS + cb0 - wb) * EB;   // offsets in a record
     unsigned tpre = t_in;                               // record counter of the prefetch
     int rpre = rho_start;                               // its iteration
-    if (nA != Cfg::COLS * 16 || nB != (Cfg::COLS + 2) * 16) {   // first / last strip of a row
-        for (int e = lane; e < DIN * REC; e += 32) sts_d2_volatile(ring + (unsigned)e * 16u, zero);
+    if (nA != Cfg::ACOLS * EB || nB != (Cfg::COLS + 2) * EB) {   // first / last strip of a row
+        for (int e = lane; e < DIN * REC * EB / 16; e += 32) sts_d2_volatile(ring + (unsigned)e * 16u, zero);
         asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");   // generic writes before the bulk copies' writes
     }
     __syncwarp();
     // Rows outside the lattice / the trapezoid are clamped to the nearest row the segment reads anyway (the record is
     // then read as zero, see `okh`, `okf` below): the prefetch is branch-free, two copies of fixed size per record.
-    const double2* gA = Hin + ca0;
-    const double2* gF = Hin + (Y + cb0);
+    const ST* gA = Hin + ca0;
+    const ST* gF = Hin + (Y + cb0);
     auto prefetch = [&]() {
         // (the record that lived in this slot was read two iterations ago: those loads have long been consumed)
         if (rpre <= rho_end && elect_one()) {
@@ -287,11 +307,11 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
     };
 #pragma unroll
     for (int v = 0; v < DPRE; ++v) prefetch();
-    const unsigned a_lane = ring + (unsigned)lane * (K * 16);                             // this lane's A columns
+    const unsigned a_lane = ring + (unsigned)(AX + K * lane) * EB;                        // this lane's A columns
 
     // ---- results -> HBM ----------------------------------------------------------------------------------
-    double2* __restrict__ Hout = state_ptr(L, nxt, 0, sys) + col0;
-    double2* __restrict__ Fout = Hout + Y;
+    ST* __restrict__ Hout = (ST*)L.state + (((size_t)nxt * 2) * L.n_batch + sys) * grid_points(L) + (size_t)GHOST * pitch + col0;
+    ST* __restrict__ Fout = Hout + Y;
 
     // partial right-hand sides in flight: tensor memory, [stage][slot] x (K pairs = 8 columns of 32 bits); the slot
     // is the parity of the iteration (a row started in iteration rho is finished in iteration rho + 2)
@@ -319,11 +339,11 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
         if (EDGE) { okh = (unsigned)(r + 2) <= (unsigned)rh_max; okf = (unsigned)(r + 1) <= (unsigned)rf_max; }
 #pragma unroll
         for (int q = 0; q < K; ++q) {
-            RA[q] = okh ? lds_d2_volatile(src + q * 16) : zero;
-            RB[q] = okf ? lds_d2_volatile(src + (Cfg::COLS + 1 + q) * 16) : zero;
+            RA[q] = okh ? lds_pair<EB>(src + q * EB) : zero;
+            RB[q] = okf ? lds_pair<EB>(src + (Cfg::ACOLS - AX + 1 + q) * EB) : zero;
         }
-        RFL = okf ? lds_d2_volatile(src + Cfg::COLS * 16) : zero;
-        RFR = okf ? lds_d2_volatile(src + (Cfg::COLS + 1 + K) * 16) : zero;
+        RFL = okf ? lds_pair<EB>(src + (Cfg::ACOLS - AX) * EB) : zero;
+        RFR = okf ? lds_pair<EB>(src + (Cfg::ACOLS - AX + 1 + K) * EB) : zero;
         ++t_in;
     };
     take(std::true_type{}, rho, false);
@@ -416,22 +436,26 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
                 }
                 const bool mine = (n >= r0 && n < r0 + Lr);
                 if (j >= NS - 2 && mine) {                            // the two newest time levels go to HBM
-                    double2* out = (j == NS - 1) ? Fout + (o_out - pitch) : Hout + o_out;
+                    ST* out = (j == NS - 1) ? Fout + (o_out - pitch) : Hout + o_out;
 #pragma unroll
                     for (int q = 0; q < K; ++q)
-                        if (own[q]) out[q] = Zo[q];
+                        if (own[q]) st_pair(out + q, Zo[q]);
                 }
                 if (EDGE && (j & 1) == 0 && mine && n <= 1) {         // whole grid of step k + j/2 + 1: reductions
                     double v = 0.0;
 #pragma unroll
                     for (int q = 0; q < K; ++q)
-                        if (own[q]) v += (n == 0) ? Zo[q].x : Zo[q].y;
+                        if (own[q]) {                                 // (fp32 storage: the stored, rounded value)
+                            const double z = (n == 0) ? Zo[q].x : Zo[q].y;
+                            v += EB == 8 ? (double)(float)z : z;
+                        }
                     accs[((j >> 1) * 2 + n) * 32 + lane] = v;
                     if (j == NS - 2 && n == 1) {
 #pragma unroll
                         for (int q = 0; q < K; ++q) {
-                            if (own[q] && col0 + q == 0) L.ss[sys].edge[0] = fabs(Zo[q].y);
-                            if (own[q] && col0 + q == L.M1 - 1) L.ss[sys].edge[1] = fabs(Zo[q].y);
+                            const double z = EB == 8 ? (double)(float)Zo[q].y : Zo[q].y;
+                            if (own[q] && col0 + q == 0) L.ss[sys].edge[0] = fabs(z);
+                            if (own[q] && col0 + q == L.M1 - 1) L.ss[sys].edge[1] = fabs(z);
                         }
                     }
                 }
@@ -494,9 +518,9 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
 }
 
 // BUDGETS: some system has a step budget (n_steps_total > 0) => the active set is compacted on the fly.
-template <int S, int K, bool BUDGETS>
-__global__ void __launch_bounds__(WarpCfg<S, K>::T, 1) warpsweep_kernel(const __grid_constant__ Layout L) {
-    using Cfg = WarpCfg<S, K>;
+template <int S, int K, bool BUDGETS, int EB>
+__global__ void __launch_bounds__(WarpCfg<S, K, EB>::T, 1) warpsweep_kernel(const __grid_constant__ Layout L) {
+    using Cfg = WarpCfg<S, K, EB>;
     constexpr int W = Cfg::W, WARPS = Cfg::WARPS, T = Cfg::T;
     static_assert(Cfg::MAX_SPAN == 64 && WARPS <= 16, "WarpShared sizes");
     extern __shared__ double2 ws_smem[];
@@ -591,7 +615,7 @@ __global__ void __launch_bounds__(WarpCfg<S, K>::T, 1) warpsweep_kernel(const __
             const int a = (int)(g / n_strips);
             const int strip = (int)(g - (long long)a * n_strips);
             const int sys = BUDGETS ? uni(sh.list[a - a_first]) : a;
-            warpsweep_segment<S, K>(L, sys, strip, r0, Lr, n_strips, ups, ring, tabp, bars, tmP, accs, t_in);
+            warpsweep_segment<S, K, EB>(L, sys, strip, r0, Lr, n_strips, ups, ring, tabp, bars, tmP, accs, t_in);
         }
     }
 

@@ -65,6 +65,63 @@ def test_fp32_modes_match_the_oracle_with_ac_field_and_budget(precision):
         s.destroy()
 
 
+@pytest.mark.parametrize("sweep_steps", [2, 3])
+@pytest.mark.parametrize("N,M1", [(40, 801), (97, 300), (33, 90)])
+def test_fp32_storage_through_the_warp_kernel(N, M1, sweep_steps):
+    """precision 1 on lattices of at least 32 rows runs the multi-step warp kernel with fp32 rows in HBM (half the bytes)
+    and fp64 arithmetic; single steps (remainders) run the two-launch form.  Inside a pass the intermediate time levels stay
+    fp64 in registers, so the result differs from the oracle (which rounds every half-update to fp32) by a few fp32 ulps of
+    max|f| -- the same bound as the two-launch form."""
+    from paper_1401_6047_b200 import Solver
+    from oracle import OracleSim
+    w = W.small_case(N=N, M1=M1, dt=0.004, n_steps=50, avg_start=7)
+    s = Solver(w.grid, w.params, precision=1)
+    s.set_option("sweep_steps", sweep_steps)
+    s.set_option("graph_steps", 0)
+    assert s.get_option("effective_variant") == 5
+    s.init_equilibrium()
+    n0 = s.launch_count()
+    s.step(17); s.step(1); s.step(32)
+    sim = OracleSim(w.grid.n_harm, w.grid.n_phiy, w.grid.dt, w.params[0], threads=4, precision=1)
+    sim.init_equilibrium()
+    sim.step(50)
+    scale = max(np.abs(x).max() for g in (0, 1) for x in sim.get_state(g))
+    for g in (0, 1):
+        a, b = s.get_state(0, g)
+        ra, rb = sim.get_state(g)
+        assert np.array_equal(a, a.astype(np.float32).astype(np.float64))          # what is stored is fp32
+        assert max(np.abs(a - ra).max(), np.abs(b - rb).max()) <= 8 * EPS32 * scale, (g,)
+        assert np.all(b[0] == 0.0)
+    o, r = s.observables()[0], sim.observables()
+    assert o.step == r.step == 50
+    assert abs(o.v_dr - r.v_dr) <= 1e-5 * max(abs(r.v_dr), 0.05) and abs(o.norm - r.norm) <= 1e-5
+    assert abs(o.sum_vcos_dt - r.sum_vcos_dt) <= 1e-5 * max(abs(r.sum_vcos_dt), 0.05 * r.window)
+    s.destroy()
+
+
+def test_fp32_storage_batch_with_budgets_through_the_warp_kernel():
+    from paper_1401_6047_b200 import Solver
+    from oracle import OracleSim
+    w = W.random_batch(n_batch=5, N=40, M1=200, dt=0.004, seed=77, periods=0.2)
+    n = w.n_steps + 4
+    s = Solver(w.grid, w.params, precision=1)
+    assert s.get_option("effective_variant") == 5
+    s.init_equilibrium()
+    s.step(n)
+    obs = s.observables()
+    for i in range(5):
+        sim = OracleSim(w.grid.n_harm, w.grid.n_phiy, w.grid.dt, w.params[i], threads=4, precision=1)
+        sim.init_equilibrium()
+        sim.step(n)
+        scale = max(np.abs(x).max() for g in (0, 1) for x in sim.get_state(g))
+        for g in (0, 1):
+            a, b = s.get_state(i, g)
+            ra, rb = sim.get_state(g)
+            assert max(np.abs(a - ra).max(), np.abs(b - rb).max()) <= 8 * EPS32 * scale, (i, g)
+        assert obs[i].step == w.params[i].n_steps_total
+    s.destroy()
+
+
 def test_fp32_state_roundtrip_and_batch():
     from paper_1401_6047_b200 import Solver
     rng = np.random.default_rng(3)
