@@ -47,7 +47,10 @@
 #define BTE_WS_K 3
 #endif
 #ifndef BTE_WS_DIN
-#define BTE_WS_DIN 8
+#define BTE_WS_DIN 4
+#endif
+#ifndef BTE_WS_TMSLOT
+#define BTE_WS_TMSLOT 0
 #endif
 #ifndef BTE_WS_COVER
 #define BTE_WS_COVER 6
@@ -77,7 +80,7 @@ struct WarpCfg {
     static constexpr int MAX_SPAN = 64;         // distinct systems one CTA range may touch
     // tensor memory: warp w owns the 32 lanes of quadrant w % 4, columns (w / 4) * TM_COLS .. + 2 NS TM_SLOT - 1;
     // one slot = the K pairs (4 K 32-bit columns, rounded to a power of two) of one stage and one iteration parity
-    static constexpr int TM_SLOT = K <= 2 ? 8 : 16;
+    static constexpr int TM_SLOT = BTE_WS_TMSLOT ? BTE_WS_TMSLOT : (K <= 2 ? 8 : 16);
     static constexpr int TM_COLS = 2 * NS * TM_SLOT;
     static constexpr int TM_NEED = ((WARPS + 3) / 4) * TM_COLS;
     static constexpr int TM_ALLOC = TM_NEED <= 32 ? 32 : TM_NEED <= 64 ? 64 : TM_NEED <= 128 ? 128 : TM_NEED <= 256 ? 256 : 512;
@@ -174,8 +177,17 @@ __device__ __forceinline__ void tm_st_d2(unsigned taddr, double2 a) {
 }
 template <int NR>
 __device__ __forceinline__ void tm_ld(unsigned taddr, unsigned (&r)[NR]) {
-    static_assert(NR == 8 || NR == 16, "x8 or x16");
-    if constexpr (NR == 8) {
+    static_assert(NR == 8 || NR == 12 || NR == 16, "x8, x8 + x4 or x16");
+    if constexpr (NR == 12) {
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n"
+                     : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                     : "r"(taddr)
+                     : "memory");
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];\n"
+                     : "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11])
+                     : "r"(taddr + 8u)
+                     : "memory");
+    } else if constexpr (NR == 8) {
         asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n"
                      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
                      : "r"(taddr)
@@ -195,6 +207,10 @@ __device__ __forceinline__ void tm_wait_ld(unsigned (&r)[NR]) {
     if constexpr (NR == 8) {
         asm volatile("tcgen05.wait::ld.sync.aligned;\n"
                      : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7])::"memory");
+    } else if constexpr (NR == 12) {
+        asm volatile("tcgen05.wait::ld.sync.aligned;\n"
+                     : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]),
+                       "+r"(r[8]), "+r"(r[9]), "+r"(r[10]), "+r"(r[11])::"memory");
     } else {
         asm volatile("tcgen05.wait::ld.sync.aligned;\n"
                      : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]),
@@ -476,7 +492,7 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
         }
         ++rho; nd0 += 1.0;
         o_out += pitch; ++cnp;
-        tmS ^= (unsigned)SL;                            // the other slot
+        tmS = tmS == tmP ? tmP + (unsigned)SL : tmP;    // the other slot
         if (EDGE) { if (rho <= rho_end) take(edge_tag, rho, landed); }
         else take(edge_tag, rho, landed);               // steady state: the next record is a full one too
     };
