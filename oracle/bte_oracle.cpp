@@ -16,8 +16,11 @@
  * the field-reversal mirror, E=0 stationarity of f0 with order-2 convergence, order-2 convergence in
  * dt, the Tucker ac averages, a dense brute-force restatement on tiny grids, checkerboard independence
  * and affinity; the reconstruction of f (eq. 8) against eq. (13) at t = 0 and against a numpy contraction; the
- * pendulum averages (eq. 44-46) against the T = 0 Esaki-Tsu and Tucker closed forms and the energy invariant.  Absolute values of configs 1-4 have no closed form and the paper prints none:
- * for those "parity unpinned" beyond the invariants listed above.
+ * pendulum averages (eq. 44-46) against the T = 0 Esaki-Tsu and Tucker closed forms and the energy invariant; the steady
+ * drift velocity in CROSSED dc fields at finite temperature against the exact solution of eq. (5) by characteristics
+ * (P12: Chambers path integral over the flow (44)-(45) with the Boltzmann f0 of eq. 13; fields of configs 1 and 4).
+ * The time-dependent (ac) absolute values of configs 1-4 have no closed form and the paper prints none: for those
+ * "parity unpinned" beyond P12 at their dc fields, P9 at B = 0 and the invariants listed above.
  *
  * Build: g++ -std=c++17 -O2 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).
  * -ffp-contract=off: no FMA contraction, every operation rounds once, in the order written.

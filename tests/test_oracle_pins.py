@@ -593,3 +593,68 @@ def test_fp32_norm_drift_grows_as_dt_shrinks():
     assert abs(_run_prec(0, 1e-4, 0.5).observables().norm - 1.0) < 1e-12
     d1 = abs(_run_prec(1, 1e-4, 0.5).observables().norm - 1.0)
     assert 1e-8 < d1 < drift[1e-4] / 10      # storage rounding alone: unbiased, a random walk -- far smaller
+
+
+# ---------------------------------------------------------------------------------------------------
+# P12: finite-temperature characteristics (Chambers path integral) -- an absolute pin for B != 0
+# ---------------------------------------------------------------------------------------------------
+def _chambers_drift_velocity(E, B, mu, nx=96, ny=160, h=0.01, s_max=24.0):
+    """Exact steady solution of eq. (5) for constant fields by the method of characteristics ("closely
+    related to the method of characteristic curves"; eq. (46) generalised from the T = 0 delta function to the Boltzmann
+    f0 of eq. (13)):  f(phi, t) = int_0^inf ds e^-s f0(phi(t - s)) along the characteristics (44)-(45), whose flow is
+    area preserving (the divergence of (E + B phi_y, -B sin phi_x) vanishes), hence
+
+        v_dr = int_0^inf ds e^-s < sin phi_x(s) >,   (phi_x, phi_y)(0) drawn from f0.
+
+    f0 factorises (eq. 13): phi_x ~ exp(mu cos phi_x), phi_y ~ N(0, 1/mu).  Both averages by the rectangle rule on uniform
+    nodes (periodic in phi_x, +-7 sigma in phi_y: spectrally accurate once the phase mixing exp(i B s phi_y) is resolved;
+    Gauss-Hermite nodes converge much more slowly here).  Trajectories by classical RK4, the s-integral by the
+    trapezoidal rule on the RK4 nodes (error ~ h^2 / 12).  Nothing of the finite-difference scheme enters.  Converged to
+    ~1e-5 (E, B, mu = 2, 1, 2) and ~5e-5 (3, 2, 1) against nx, ny = 128, 256, h = 0.005."""
+    px = -np.pi + 2 * np.pi * (np.arange(nx) + 0.5) / nx
+    wx = np.exp(mu * (np.cos(px) - 1.0)); wx /= wx.sum()
+    ymax = 7.0 / math.sqrt(mu)
+    py = -ymax + 2 * ymax * (np.arange(ny) + 0.5) / ny
+    wy = np.exp(-0.5 * mu * py * py); wy /= wy.sum()
+    X, Y = np.meshgrid(px, py, indexing="ij")
+    Wt = wx[:, None] * wy[None, :]
+
+    def rhs(x, y):
+        return E + B * y, -B * np.sin(x)
+
+    n = int(round(s_max / h))
+    acc = 0.5 * np.sum(Wt * np.sin(X))                     # trapezoid: half weight at s = 0
+    for k in range(1, n + 1):
+        k1x, k1y = rhs(X, Y)
+        k2x, k2y = rhs(X + 0.5 * h * k1x, Y + 0.5 * h * k1y)
+        k3x, k3y = rhs(X + 0.5 * h * k2x, Y + 0.5 * h * k2y)
+        k4x, k4y = rhs(X + h * k3x, Y + h * k3y)
+        X = X + h / 6.0 * (k1x + 2 * k2x + 2 * k3x + k4x)
+        Y = Y + h / 6.0 * (k1y + 2 * k2y + 2 * k3y + k4y)
+        acc += (0.5 if k == n else 1.0) * math.exp(-k * h) * np.sum(Wt * np.sin(X))
+    return acc * h
+
+
+def test_P12_chambers_integral_reduces_to_esaki_tsu_at_B0():
+    """The validator itself, pinned: at B = 0 the path integral is (I1/I0) E / (1 + E^2) in closed form."""
+    E, mu = 1.3, 2.0
+    ref = special.iv(1, mu) / special.iv(0, mu) * E / (1.0 + E * E)
+    assert abs(_chambers_drift_velocity(E, 0.0, mu, nx=64, ny=16, h=0.01) - ref) < 2e-5    # trapezoid in s: O(h^2)
+
+
+@pytest.mark.parametrize("E,B,mu,N,M1,dt", [(2.0, 1.0, 2.0, 40, 401, 0.004),      # config 1's fields, dc part
+                                            (3.0, 2.0, 1.0, 48, 481, 0.004)])     # config 4's fields, dc part
+def test_P12_steady_drift_velocity_in_crossed_fields_matches_the_characteristics(E, B, mu, N, M1, dt):
+    """Absolute pin at B != 0: the oracle's steady v_dr in crossed dc fields at finite temperature against
+    the exact solution of eq. (5) by characteristics.  Every term of eq. (30)-(33) takes part (the phi_y stencil with
+    its signs and chi(1) = 2, the rotation n (E + B phi_y), the relaxation), so a dropped term, a wrong sign or a
+    transposed index moves v_dr by far more than the 5e-4 asked for (the discretisation error is O(dt^2 + dphi^2))."""
+    ymax = W.phiy_extent(mu, E, 0.0, B, dt, M1)
+    s, p = make(N, M1, dt, E_dc=E, B=B, mu=mu, phiy_min=-ymax, phiy_max=ymax)
+    s.threads = 4
+    s.init_equilibrium()
+    s.step(int(round(24.0 / dt)))
+    o = s.observables()
+    ref = _chambers_drift_velocity(E, B, mu)
+    assert abs(o.norm - 1.0) < 1e-10 and o.edge_leak < 1e-12
+    assert abs(o.v_dr - ref) < 5e-4 * max(abs(ref), 0.05), (o.v_dr, ref)
