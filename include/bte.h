@@ -218,6 +218,23 @@ BTE_API int bte_set_option(bte_ctx* ctx, const char* key, int64_t value);
  * the device that owns the workspace; every entry point selects it and restores the caller's device).           */
 BTE_API int bte_get_option(bte_ctx* ctx, const char* key, int64_t* out /* host */);
 
+/* Steady-state detection and averaging policy, evaluated on the device after every time step ("let the
+ * system relax" to t = 10, "then compute averages over the period 2 pi / omega"; C23).
+ * Per system: P = round(2 pi / (omega dt)) steps is one ac period (omega = 0: P = round(1 / dt), one relaxation time).
+ * After every interval of P steps the mean drift velocity m_i of that interval is compared with m_{i-1}; the system
+ * counts as relaxed when i >= max(2, min_relax_periods) and |m_i - m_{i-1}| <= rel_tol * max(|m_i|, |m_{i-1}|, 1e-3).
+ * From the next step on sum_v_dt, sum_vcos_dt, sum_vsin_dt and window of bte_obs run for exactly
+ * round(n_avg_periods * 2 pi / (omega dt)) steps (rounded once for the whole window); then the system is FINISHED: its observables are final and later launches do not advance it (bte_obs.step says
+ * where it stopped, at most a launch group beyond the window).  params.avg_start_step is ignored while the policy is on,
+ * params.n_steps_total still ends a system.  rel_tol = 0 switches the policy off (default).  Call before
+ * bte_init_equilibrium.  Streaming sweep kernels only (fp64, variant 0, 3 or 5; the resident kernel is not used):
+ * BTE_EINVAL otherwise.                                                                                          */
+BTE_API int bte_set_steady_policy(bte_ctx* ctx, double rel_tol, int32_t n_avg_periods, int32_t min_relax_periods);
+
+/* Per system: the step at which it was found relaxed (0 = not yet) and its phase (0 relaxing, 1 averaging, 2 finished).
+ * Synchronises the stream.  steady_step, phase: host, n_batch entries each.                                      */
+BTE_API int bte_steady_info(bte_ctx* ctx, int64_t* steady_step /* host */, int32_t* phase /* host */);
+
 /* Number of kernel launches (graph nodes counted individually) issued by this ctx so far. */
 BTE_API int bte_launch_count(bte_ctx* ctx, int64_t* out /* host */);
 

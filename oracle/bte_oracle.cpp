@@ -51,6 +51,12 @@ struct Sim {
     std::vector<float> cf, gf;          /* precision 2: c_n and g_m = exp(-mu phi^2/2) rounded to fp32   */
     int64_t step;
     double norm, v_dr, sum_v, sum_c, sum_s, window;
+    /* steady-state detection and averaging policy (C23); steady_tol = 0: off */
+    double steady_tol;
+    int n_avg_periods, min_relax_periods;
+    int64_t period_steps, window_steps, interval_pos, intervals_done, window_left, steady_step;
+    double interval_sum, previous_mean;
+    int phase;              /* 0 relaxing, 1 averaging, 2 finished */
     int threads;
     int precision;          /* 0: fp64 (default); 1: state stored as fp32, arithmetic fp64; 2: fp32 throughout (NEXT-4) */
 };
@@ -230,6 +236,9 @@ void* oracle_create(int32_t n_harm, int32_t n_phiy, double dt, const oracle_para
     s->n_steps_total = p->n_steps_total; s->avg_start_step = p->avg_start_step;
     s->threads = threads > 0 ? threads : 1;
     s->precision = 0;
+    s->steady_tol = 0.0; s->n_avg_periods = 0; s->min_relax_periods = 0; s->period_steps = 0; s->window_steps = 0;
+    s->interval_pos = s->intervals_done = s->window_left = s->steady_step = 0;
+    s->interval_sum = s->previous_mean = 0.0; s->phase = 0;
     fill_equilibrium(s);
     const size_t P = (size_t)(s->N + 1) * s->M1;
     s->ha.assign(P, 0.0); s->hb.assign(P, 0.0); s->fa.assign(P, 0.0); s->fb.assign(P, 0.0);
@@ -292,7 +301,37 @@ void oracle_step(void* h, int64_t n_steps, double* v_trace, double* norm_trace) 
         s->step += 1;
         const double t = (double)s->step * s->dt;
         reduce_observables(s);
-        if (s->step > s->avg_start_step) {
+        bool accumulate = s->step > s->avg_start_step;          /* fixed window, reading C9 */
+        if (s->steady_tol > 0.0) {
+            /* Reading C23 of PAPER.md:L103 ("let the system relax ... then compute averages over the period"): the mean
+             * drift velocity of every interval of P steps (one ac period) is compared with that of the interval
+             * before; once two consecutive means agree to steady_tol (not before max(2, min_relax) intervals) the sums
+             * of eq. (17) run over the next round(n_avg_periods * period / dt) steps, then stop for good. */
+            accumulate = false;
+            if (s->phase == 1) {
+                accumulate = true;
+                s->window_left -= 1;
+                if (s->window_left == 0) s->phase = 2;
+            } else if (s->phase == 0) {
+                s->interval_sum += s->v_dr;
+                s->interval_pos += 1;
+                if (s->interval_pos == s->period_steps) {
+                    const double mean = s->interval_sum / (double)s->period_steps;
+                    s->intervals_done += 1;
+                    const double scale = std::max(std::max(std::fabs(mean), std::fabs(s->previous_mean)), 1e-3);
+                    const int64_t need = std::max(2, s->min_relax_periods);
+                    if (s->intervals_done >= need && std::fabs(mean - s->previous_mean) <= s->steady_tol * scale) {
+                        s->phase = 1;
+                        s->window_left = s->window_steps;
+                        s->steady_step = s->step;
+                    }
+                    s->previous_mean = mean;
+                    s->interval_sum = 0.0;
+                    s->interval_pos = 0;
+                }
+            }
+        }
+        if (accumulate) {
             s->sum_v += s->v_dr * s->dt;
             s->sum_c += s->v_dr * std::cos(s->omega * t) * s->dt;
             s->sum_s += s->v_dr * std::sin(s->omega * t) * s->dt;
@@ -301,6 +340,26 @@ void oracle_step(void* h, int64_t n_steps, double* v_trace, double* norm_trace) 
         if (v_trace) v_trace[j] = s->v_dr;
         if (norm_trace) norm_trace[j] = s->norm;
     }
+}
+
+/* Switch the steady-state policy on (tol > 0) or off; resets its bookkeeping.  P = one ac period in steps, or one
+ * relaxation time for a dc system.  (A finished system keeps evolving when stepped; only its sums are final.) */
+void oracle_set_steady_policy(void* h, double tol, int32_t n_avg_periods, int32_t min_relax_periods) {
+    Sim* s = (Sim*)h;
+    const double pi = 3.14159265358979323846;
+    const double w = std::fabs(s->omega);
+    const double P = w > 0.0 ? 2.0 * pi / (w * s->dt) : 1.0 / s->dt;
+    s->period_steps = std::max<int64_t>(1, std::llround(P));
+    s->window_steps = std::max<int64_t>(1, std::llround((double)n_avg_periods * P));   /* rounded once, not per period */
+    s->steady_tol = tol; s->n_avg_periods = n_avg_periods; s->min_relax_periods = min_relax_periods;
+    s->interval_pos = 0; s->intervals_done = 0; s->window_left = 0; s->steady_step = 0;
+    s->interval_sum = 0.0; s->previous_mean = 0.0; s->phase = 0;
+}
+
+void oracle_steady_info(void* h, int64_t* steady_step, int32_t* phase) {
+    Sim* s = (Sim*)h;
+    *steady_step = s->steady_step;
+    *phase = s->phase;
 }
 
 void oracle_observables(void* h, oracle_obs* o) {

@@ -58,6 +58,8 @@ def _load():
         lib.oracle_reconstruct_pdf.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
         lib.oracle_pendulum_averages.argtypes = [C.c_double] * 4 + [C.c_int32, C.c_double, C.c_int32, C.c_void_p]
         lib.oracle_pendulum_trajectory.argtypes = [C.c_double] * 6 + [C.c_int32, C.c_void_p, C.c_void_p]
+        lib.oracle_set_steady_policy.argtypes = [C.c_void_p, C.c_double, C.c_int32, C.c_int32]
+        lib.oracle_steady_info.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int32)]
         lib.oracle_max_threads.restype = C.c_int32
         _lib = lib
     return _lib
@@ -109,6 +111,15 @@ class OracleSim:
 
     def init_equilibrium(self):
         _load().oracle_init_equilibrium(self._h)
+
+    def set_steady_policy(self, rel_tol: float, n_avg_periods: int, min_relax_periods: int = 0):
+        """Steady-state detection and averaging policy (C23); rel_tol = 0 switches it off."""
+        _load().oracle_set_steady_policy(self._h, float(rel_tol), int(n_avg_periods), int(min_relax_periods))
+
+    def steady_info(self):
+        st, ph = C.c_int64(), C.c_int32()
+        _load().oracle_steady_info(self._h, C.byref(st), C.byref(ph))
+        return int(st.value), int(ph.value)
 
     def startup_from_whole(self):
         _load().oracle_startup_from_whole(self._h)

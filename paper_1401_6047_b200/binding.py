@@ -23,7 +23,7 @@ EXPORTS = ("bte_workspace_bytes", "bte_create", "bte_init_equilibrium", "bte_ste
            "bte_reconstruct_pdf", "bte_pendulum_workspace_bytes",
            "bte_pendulum_averages", "bte_rs_workspace_bytes", "bte_rs_create", "bte_rs_init_equilibrium",
            "bte_rs_step", "bte_rs_observables", "bte_rs_get_state", "bte_rs_destroy", "bte_set_option",
-           "bte_launch_count",
+           "bte_launch_count", "bte_set_steady_policy", "bte_steady_info",
            "bte_last_error")
 
 
@@ -97,6 +97,10 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     for name in ("bte_get_state_batch", "bte_set_state_batch"):
         getattr(lib, name).restype = C.c_int
         getattr(lib, name).argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+    lib.bte_set_steady_policy.restype = C.c_int
+    lib.bte_set_steady_policy.argtypes = [C.c_void_p, C.c_double, C.c_int32, C.c_int32]
+    lib.bte_steady_info.restype = C.c_int
+    lib.bte_steady_info.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int32)]
     lib.bte_get_option.restype = C.c_int
     lib.bte_get_option.argtypes = [C.c_void_p, C.c_char_p, C.POINTER(C.c_int64)]
     lib.bte_reconstruct_pdf.restype = C.c_int
@@ -330,6 +334,17 @@ class Solver:
         v = C.c_int64()
         _check(self._lib.bte_get_option(self._h, key.encode(), C.byref(v)))
         return int(v.value)
+
+    def set_steady_policy(self, rel_tol: float, n_avg_periods: int, min_relax_periods: int = 0):
+        _check(self._lib.bte_set_steady_policy(self._h, float(rel_tol), int(n_avg_periods), int(min_relax_periods)))
+
+    def steady_info(self):
+        """(steady_step, phase) per system."""
+        nb = self.grid.n_batch
+        st = (C.c_int64 * nb)()
+        ph = (C.c_int32 * nb)()
+        _check(self._lib.bte_steady_info(self._h, st, ph))
+        return list(st), list(ph)
 
     def launch_count(self) -> int:
         n = C.c_int64()

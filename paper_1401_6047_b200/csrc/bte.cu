@@ -158,6 +158,8 @@ struct bte_ctx {
     int ws_grid[SWEEP_MAX_STEPS + 1];   // same for the warp kernel (bte_warpsweep.cuh), S = 2 .. WS_MAX_STEPS
     int sm_count;
     std::vector<int64_t> budgets;    // sorted distinct step budgets (n_steps_total > 0)
+    std::vector<SysConst> sc_host;   // host copy of the per-system constants (re-uploaded by bte_set_steady_policy)
+    bool steady_on;                  // steady-state detection / averaging policy in force
     // resident (on-chip) kernel launch plan
     int res_ctas_opt;                // option: slabs (0 = automatic)
     int res_mode;                    // -1 = not usable; 0 one CTA, 1 one cluster, 2 cooperative grid
@@ -716,6 +718,7 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
         k.norm_scale = 2.0 * PI * std::sqrt(p.alpha) * dphi;
         k.v_scale = PI * std::sqrt(p.alpha) * dphi;
         k.n_steps_total = p.n_steps_total; k.avg_start_step = p.avg_start_step;
+        k.period_steps = 0; k.window_steps = 0; k.steady_tol = 0.0; k.n_avg_periods = 0; k.min_relax_periods = 0;
     }
     char* ws = (char*)workspace;
     CUDA_TRY(cudaMemcpyAsync(ws + off.cn, cn.data(), cn.size() * sizeof(double), cudaMemcpyHostToDevice, stream));
@@ -744,6 +747,7 @@ int bte_create(const bte_grid* grid, const bte_params* params, void* workspace, 
     c->L.partial = (double*)(ws + off.partial);
     c->L.gctl = (unsigned int*)(ws + off.gctl);
     c->has_budgets = false;
+    c->sc_host = sc; c->steady_on = false;
     for (int s = 0; s < nb; ++s) c->has_budgets = c->has_budgets || params[s].n_steps_total > 0;
     for (int s = 0; s < nb; ++s)
         if (params[s].n_steps_total > 0) c->budgets.push_back(params[s].n_steps_total);
@@ -803,7 +807,7 @@ int bte_step(bte_ctx* c, int64_t n_steps) {
     // (batches: only small systems -- a batch of mid-size systems streams faster through the sweep kernel)
     const bool res_auto = c->variant == VAR_AUTO && n_steps >= 4 &&
                           (c->grid.n_batch == 1 || (long long)(c->grid.n_harm + 1) * c->grid.n_phiy <= RES_BATCH_MAX_POINTS);
-    if (c->res_mode >= 0 && (c->variant == VAR_RESIDENT || res_auto)) {
+    if (c->res_mode >= 0 && (c->variant == VAR_RESIDENT || res_auto) && !c->steady_on) {
         int64_t n = n_steps;
         if (c->grid.n_batch == 1) {            // (a batch: the kernel ends every system at its own budget)
             const int64_t tot = c->params[0].n_steps_total;
@@ -1026,6 +1030,48 @@ int bte_set_state_batch(bte_ctx* c, int32_t grid_id, const double* a, const doub
     }
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return BTE_OK;
+}
+
+int bte_set_steady_policy(bte_ctx* c, double rel_tol, int32_t n_avg_periods, int32_t min_relax_periods) {
+    if (!c) return fail(BTE_EINVAL, "bte_set_steady_policy: NULL context");
+    CTX_GUARD(c);
+    if (!(rel_tol >= 0.0) || !std::isfinite(rel_tol) || (rel_tol > 0.0 && (n_avg_periods < 1 || min_relax_periods < 0)))
+        return fail(BTE_EINVAL, "bte_set_steady_policy: need rel_tol >= 0, n_avg_periods >= 1, min_relax_periods >= 0");
+    if (rel_tol > 0.0) {
+        const int var = effective_variant(c);
+        if (c->grid.precision != 0 || !is_sweep(var))
+            return fail(BTE_EINVAL, "bte_set_steady_policy: runs in the streaming sweep kernels only (fp64, variant 0, 3 or 5)");
+    }
+    const double PI = 3.14159265358979323846;
+    for (size_t s = 0; s < c->sc_host.size(); ++s) {
+        SysConst& k = c->sc_host[s];
+        const double w = std::fabs(c->params[s].omega);
+        // comparison interval: one ac period; a dc system (omega = 0): one relaxation time (C23)
+        const double P = w > 0.0 ? 2.0 * PI / (w * c->grid.dt) : 1.0 / c->grid.dt;
+        k.period_steps = std::max<long long>(1, std::llround(P));
+        k.window_steps = std::max<long long>(1, std::llround((double)n_avg_periods * P));
+        k.steady_tol = rel_tol; k.n_avg_periods = n_avg_periods; k.min_relax_periods = min_relax_periods;
+    }
+    CUDA_TRY(cudaMemcpyAsync(c->ws + c->off.sc, c->sc_host.data(), c->sc_host.size() * sizeof(SysConst),
+                             cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    const bool was = c->has_budgets;
+    c->steady_on = rel_tol > 0.0;
+    // finished systems are compacted out of the launches like systems past their budget
+    c->has_budgets = c->steady_on;
+    for (size_t s = 0; s < c->params.size(); ++s) c->has_budgets = c->has_budgets || c->params[s].n_steps_total > 0;
+    if (was != c->has_budgets) { drop_graph(c); return plan_sweep(c); }
+    return BTE_OK;
+}
+
+int bte_steady_info(bte_ctx* c, int64_t* steady_step, int32_t* phase) {
+    if (!c || !steady_step || !phase) return fail(BTE_EINVAL, "bte_steady_info: NULL argument");
+    CTX_GUARD(c);
+    std::vector<SysState> ss((size_t)c->grid.n_batch);
+    CUDA_TRY(cudaMemcpyAsync(ss.data(), c->ws + c->off.ss, ss.size() * sizeof(SysState), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    for (int s = 0; s < c->grid.n_batch; ++s) { steady_step[s] = ss[s].steady_step; phase[s] = ss[s].phase; }
     return BTE_OK;
 }
 

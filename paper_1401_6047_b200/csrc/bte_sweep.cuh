@@ -52,7 +52,7 @@ struct SweepCfg {
 // while a system has fewer than S but more than 0 steps left, bte.cu)
 __device__ __forceinline__ bool sys_active(const Layout& L, int s, int S) {
     const long long tot = L.sc[s].n_steps_total;
-    return tot == 0 || L.ss[s].k + S <= tot;
+    return (tot == 0 || L.ss[s].k + S <= tot) && L.ss[s].phase != 2;   // (phase 2: finished by the steady-state policy)
 }
 
 __device__ __forceinline__ void cp_async16_sz(unsigned smem_addr, const void* gmem_src, int src_bytes) {
@@ -113,16 +113,7 @@ __device__ __forceinline__ void fold_sweep(const Layout& L, int sys, int n_parti
             const double v = c.v_scale * sb;
             st->norm = norm;
             st->v_dr = v;
-            const long long k1 = k + s + 1;
-            if (k1 > c.avg_start_step) {
-                const double t = (double)k1 * L.dt;
-                double sn, cs;
-                sincos(c.omega * t, &sn, &cs);
-                st->sum_v += v * L.dt;
-                st->sum_c += v * cs * L.dt;
-                st->sum_s += v * sn * L.dt;
-                st->window += L.dt;
-            }
+            accumulate_step(c, st, v, k + s + 1, L.dt);
         }
     }
     if (lane == 0) {
@@ -493,7 +484,10 @@ __global__ void __launch_bounds__(T, MINB) sweep_kernel(const __grid_constant__ 
     if (sh.flag) {
         __threadfence();
         for (int s = i; s < L.n_batch; s += T)
-            if (sys_active(L, s, S)) { L.ss[s].k += S; L.ss[s].buf ^= 1; }
+            if (sys_active(L, s, S)) {
+                L.ss[s].k += S; L.ss[s].buf ^= 1;
+                if (L.ss[s].phase == 3) L.ss[s].phase = 2;
+            }
         if (i == 0) *L.gctl = 0u;
     }
 }

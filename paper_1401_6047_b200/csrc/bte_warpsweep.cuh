@@ -650,7 +650,10 @@ __global__ void __launch_bounds__(WarpCfg<S, K, EB>::T, 1) warpsweep_kernel(cons
     if (sh.flag) {
         __threadfence();
         for (int s = i; s < L.n_batch; s += T)
-            if (sys_active(L, s, S)) { L.ss[s].k += S; L.ss[s].buf ^= 1; }
+            if (sys_active(L, s, S)) {
+                L.ss[s].k += S; L.ss[s].buf ^= 1;
+                if (L.ss[s].phase == 3) L.ss[s].phase = 2;
+            }
         if (i == 0) *L.gctl = 0u;
     }
 }

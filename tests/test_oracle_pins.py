@@ -658,3 +658,93 @@ def test_P12_steady_drift_velocity_in_crossed_fields_matches_the_characteristics
     ref = _chambers_drift_velocity(E, B, mu)
     assert abs(o.norm - 1.0) < 1e-10 and o.edge_leak < 1e-12
     assert abs(o.v_dr - ref) < 5e-4 * max(abs(ref), 0.05), (o.v_dr, ref)
+
+
+# ---------------------------------------------------------------------------------------------------
+# NEXT-1: steady-state detection and averaging policy (C23)
+# ---------------------------------------------------------------------------------------------------
+def _tucker_averages(E_dc, E_w, w, mu, nmax=40):
+    """<v> and <v cos wt> of eq. (42)-(43) in the normalisation of C9."""
+    beta = E_w / w
+    r = special.iv(1, mu) / special.iv(0, mu)
+    n = np.arange(-nmax, nmax + 1)
+    xi = (E_dc + n * w) / (1.0 + (E_dc + n * w) ** 2)
+    J = special.jv(n, beta)
+    return r * np.sum(J * J * xi), 0.5 * r * np.sum(J * (special.jv(n + 1, beta) + special.jv(n - 1, beta)) * xi)
+
+
+def test_steady_policy_gives_the_tucker_averages_without_a_hand_set_window():
+    """B = 0, Fig. 3-like fields: the policy finds the relaxed state by itself and averages an integer number of
+    periods; the result is the closed form of eq. (42)-(43) (P9 reaches the same with a hand-set window)."""
+    E_dc, E_w, w, mu, dt = 2.0, 0.5, 1.5, 2.0, 0.002
+    s, p = make(2, 41, dt, E_dc=E_dc, E_omega=E_w, omega=w, mu=mu, phiy_min=-6.0, phiy_max=6.0)
+    s.set_steady_policy(1e-7, 3, 0)
+    s.init_equilibrium()
+    s.step(40000)
+    step, phase = s.steady_info()
+    o = s.observables()
+    P = round(2 * math.pi / (w * dt))
+    assert phase == 2 and step > 0 and step % P == 0
+    assert abs(o.window - round(3 * 2 * math.pi / (w * dt)) * dt) < 1e-9
+    v, vc = _tucker_averages(E_dc, E_w, w, mu)
+    assert abs(o.sum_v_dt / o.window - v) < 2e-4 * abs(v)
+    assert abs(o.sum_vcos_dt / o.window - vc) < 2e-3 * abs(vc) + 1e-6
+    # finished: the sums are final however long the system is stepped
+    before = (o.sum_v_dt, o.sum_vcos_dt, o.sum_vsin_dt, o.window)
+    s.step(777)
+    o2 = s.observables()
+    assert (o2.sum_v_dt, o2.sum_vcos_dt, o2.sum_vsin_dt, o2.window) == before and o2.step == 40777
+
+
+def test_steady_policy_detection_time_follows_the_relaxation_law():
+    """Relaxation-time scattering: the transient decays like e^{-t} (tau = 1), so tightening the tolerance by a factor
+    F delays the detection by ln F, up to the granularity of one comparison interval."""
+    E_dc, E_w, w, mu, dt = 3.0, 0.3, 4.0, 1.0, 0.004
+    P = round(2 * math.pi / (w * dt))
+    t = {}
+    for tol in (1e-3, 1e-6):
+        s, p = make(16, 11, dt, E_dc=E_dc, E_omega=E_w, omega=w, mu=mu, phiy_min=-6.0, phiy_max=6.0)
+        s.set_steady_policy(tol, 1, 0)
+        s.init_equilibrium()
+        s.step(12000)
+        step, phase = s.steady_info()
+        assert phase == 2 and step % P == 0
+        t[tol] = step * dt
+    assert abs((t[1e-6] - t[1e-3]) - math.log(1e3)) <= 1.5 * P * dt, t
+
+
+def test_steady_policy_window_equals_a_hand_set_window_bit_for_bit():
+    """The accumulation itself is the pinned one (P9): a second run with avg_start_step = detected step and a budget at
+    the end of the window gives the same sums to the last bit.  Also: a dc system compares intervals of one relaxation
+    time, min_relax_periods delays the detection, tol = 0 switches the policy off."""
+    kw = dict(E_dc=1.5, E_omega=0.4, omega=2.5, B=1.0, mu=2.0, phiy_min=-8.0, phiy_max=8.0)
+    dt = 0.005
+    s, p = make(14, 81, dt, **kw)
+    s.set_steady_policy(1e-5, 2, 0)
+    s.init_equilibrium()
+    s.step(9000)
+    step, phase = s.steady_info()
+    assert phase == 2
+    o = s.observables()
+    P = round(2 * math.pi / (2.5 * dt))
+    s2, _ = make(14, 81, dt, n_steps_total=step + round(2 * 2 * math.pi / (2.5 * dt)), avg_start_step=step, **kw)
+    s2.init_equilibrium()
+    s2.step(9000)
+    o2 = s2.observables()
+    assert (o.sum_v_dt, o.sum_vcos_dt, o.sum_vsin_dt, o.window) == (o2.sum_v_dt, o2.sum_vcos_dt, o2.sum_vsin_dt, o2.window)
+    s3, _ = make(14, 81, dt, **kw)
+    s3.set_steady_policy(1e-5, 2, 12)
+    s3.init_equilibrium()
+    s3.step(9000)
+    assert s3.steady_info() == (12 * P, 2) and 12 * P > step
+    sd, _ = make(6, 11, dt, E_dc=1.0, mu=1.0)
+    sd.set_steady_policy(1e-6, 1, 0)
+    sd.init_equilibrium()
+    sd.step(6000)
+    st_dc, ph_dc = sd.steady_info()
+    assert ph_dc == 2 and st_dc % round(1.0 / dt) == 0 and abs(sd.observables().window - 1.0) < 1e-9
+    s4, _ = make(6, 11, dt, avg_start_step=10, **kw)
+    s4.set_steady_policy(0.0, 1, 0)
+    s4.init_equilibrium()
+    s4.step(50)
+    assert s4.steady_info() == (0, 0) and abs(s4.observables().window - 40 * dt) < 1e-12
