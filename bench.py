@@ -274,7 +274,9 @@ class Ctx:
         import torch.distributed as dist
         self.torch, self.dist = torch, dist
         self.rank, self.world, self.local = dist_env()
-        if self.world > 1:
+        # under torchrun (RANK set) the NCCL process group is brought up even for a single rank, so that the barrier and
+        # the max-over-ranks reduction of the timing run through NCCL exactly as they do for N > 1
+        if self.world > 1 or os.environ.get("RANK") is not None:
             dist.init_process_group("nccl", device_id=torch.device(f"cuda:{self.local}"))
         torch.cuda.set_device(self.local)
         self.dev = f"cuda:{self.local}"
@@ -282,7 +284,7 @@ class Ctx:
         self.sampler = ClockSampler(self.local) if self.rank == 0 else None
 
     def barrier(self):
-        if self.world > 1:
+        if self.dist.is_initialized():
             self.dist.barrier()
         self.torch.cuda.synchronize()
 
@@ -491,7 +493,7 @@ def run_ours(args):
             configs[wi.name] = r
 
     if cx.rank != 0:
-        if cx.world > 1:
+        if cx.dist.is_initialized():
             cx.dist.destroy_process_group()
         return 0
 
@@ -527,7 +529,7 @@ def run_ours(args):
     if cx.world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(W.get(args.workload))
     print(json.dumps(line), flush=True)
-    if cx.world > 1:
+    if cx.dist.is_initialized():
         cx.dist.destroy_process_group()
     return 0
 

@@ -50,7 +50,7 @@ def shard_workload(w: W.Workload, rank: int, world: int) -> W.Workload:
 def barrier(sync_device=None) -> None:
     """dist.barrier() (if a process group exists) followed by a device synchronise."""
     import torch.distributed as dist
-    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+    if dist.is_available() and dist.is_initialized():
         dist.barrier()
     if sync_device is not None:
         import torch
@@ -60,7 +60,7 @@ def barrier(sync_device=None) -> None:
 def max_over_ranks(x: float, device="cpu") -> float:
     import torch
     import torch.distributed as dist
-    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+    if not (dist.is_available() and dist.is_initialized()):
         return float(x)
     t = torch.tensor([x], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -70,7 +70,7 @@ def max_over_ranks(x: float, device="cpu") -> float:
 def sum_over_ranks(x: float, device="cpu") -> float:
     import torch
     import torch.distributed as dist
-    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+    if not (dist.is_available() and dist.is_initialized()):
         return float(x)
     t = torch.tensor([x], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.SUM)
