@@ -100,11 +100,15 @@ __device__ __forceinline__ void fold_sweep(const Layout& L, int sys, int n_parti
     const SysConst c = L.sc[sys];
     SysState* st = L.ss + sys;
     for (int s = 0; s < S; ++s) {
-        const volatile double* part = L.partial + ((size_t)s * L.n_batch + sys) * L.pitch * 2;
+        // (the fold of the last system is the very end of a launch: the partial sums are read from L2 with independent
+        // 128-bit loads, several in flight, not one dependent round trip per value)
+        const double2* part = (const double2*)(L.partial + ((size_t)s * L.n_batch + sys) * L.pitch * 2);
         double sa = 0.0, sb = 0.0;
+#pragma unroll 4
         for (int p = lane; p < n_partials; p += 32) {
-            sa += part[2 * p];
-            sb += part[2 * p + 1];
+            const double2 v = __ldcg(part + p);
+            sa += v.x;
+            sb += v.y;
         }
         sa = warp_sum(sa);
         sb = warp_sum(sb);
