@@ -176,7 +176,8 @@ class ClockSampler:
         for _, _, r in self.samples:
             mask |= r
         reasons = sorted(v for k, v in self.REASONS.items() if mask & k) if reasons_smi is None else reasons_smi
-        out = {"sm_mhz": statistics.median(x[0] for x in self.samples), "sm_max_mhz": self.sm_max,
+        out = {"sm_mhz": statistics.median(x[0] for x in self.samples), "sm_mhz_min": min(x[0] for x in self.samples),
+               "sm_max_mhz": self.sm_max,
                "power_w_max": max(x[1] for x in self.samples), "samples": len(self.samples), "reasons": reasons,
                "how": "NVML in-process, ~2 ms period, inside the timed blocks only" if self._h is not None else
                       "nvidia-smi -lms 20 for the whole run"}
