@@ -25,12 +25,14 @@
  *     (the layout of Fig. 7).  Inside the workspace the state is stored as interleaved (a,b)
  *     pairs.
  *   - fp64 throughout unless bte_grid.precision asks for one of the fp32 variants of the step (the paper's own
- *     precision; reference-grade kernels).  Work is issued asynchronously on the CUDA stream given at create
+ *     precision).  Work is issued asynchronously on the CUDA stream given at create
  *     time (a cudaStream_t passed as void*; NULL = legacy default stream).
  *   - How a step is executed is chosen automatically (bte_set_option "variant"): lattices that fit the GPU's
  *     shared memory run the whole time loop of a bte_step call in one launch (resident kernel); larger ones and
- *     batches stream through HBM once per 2-3 time steps (sweep kernel).  Results do not depend on the choice
- *     beyond rounding of the sums (the state is bit-identical across variants).
+ *     batches stream through HBM once per 3 time steps (warp kernel; columns shorter than 32 rows: the
+ *     shared-memory-ring kernel, 2 steps).  Results do not depend on the choice beyond rounding: the state is
+ *     bit-identical across variants 1-4 and agrees with variant 5 to 1e-14 max|f| (variant 5 forms n beta dt/2 with
+ *     one fused multiply-add more).
  *   - Beyond the time step: bte_reconstruct_pdf (eq. 8) and bte_pendulum_averages (eq. 44-46), see below.
  *   - A ctx belongs to the CUDA device that owns its workspace: every entry point selects that device for the
  *     duration of the call and restores the caller's current device.
@@ -189,12 +191,13 @@ BTE_API int bte_rs_destroy(bte_rs_ctx* ctx);
 /* Tuning / variant selection, before or between bte_step calls.  Keys:
  *   "variant"      0 = automatic (default), 1 = two half-update kernels per step (96 B/point/step),
  *                  2 = fused whole+fractional kernel on a 2-D tile grid (64 B/point/step),
- *                  3 = persistent sweep kernel, S steps per launch (64/S B/point/step; the default path
- *                      for lattices larger than the GPU's shared memory; intermediate time levels in shared-memory
- *                      rings, one thread per phi_y column),
- *                  5 = register-pipelined sweep kernel, S = 2..4 steps per launch (same traffic; one warp per
- *                      leap-frog step, rows handed from warp to warp through per-lane shared-memory FIFOs, input rows
- *                      by TMA bulk copies; one-step launches fall back to variant 3),
+ *                  3 = persistent sweep kernel, S steps per launch (64/S B/point/step; intermediate time levels in
+ *                      shared-memory rings, one thread per phi_y column; the one-step, HBM-bound form and the
+ *                      default for columns shorter than 32 rows),
+ *                  5 = warp kernel, S = 2 or 3 steps per launch (same traffic; the default path for lattices larger
+ *                      than the GPU's shared memory and for batches: one warp per strip of 96 columns runs all 2 S
+ *                      half-updates in registers, rows in flight in tensor memory, input rows by 1-D TMA bulk copies;
+ *                      one-step launches fall back to variant 3; also bte_grid.precision 1),
  *                  4 = resident kernel: the whole time loop of one bte_step call in ONE launch, state held
  *                      in shared memory (one system: both grids must fit the shared memory of the GPU; a batch:
  *                      each system must fit one cluster of 16 CTAs; otherwise variant 3 runs).  Automatic

@@ -40,6 +40,9 @@
 
 #include "bte_sweep.cuh"
 
+// Tuning constants (compile-time; the defaults are the measured optimum on B200, DESIGN.md 5.1a / section 10):
+//   WARPS 8 (two per SMSP: 254 registers each), K 3 columns per lane, DIN 4 ring slots, CG 3 stages per coefficient
+//   group, COVER 6 (a segment is charged COVER * NS / 2 = 3 NS row-iterations in the partition), TMSLOT 0 = automatic
 #ifndef BTE_WS_WARPS
 #define BTE_WS_WARPS 8
 #endif
@@ -367,9 +370,7 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
     // edge_tag: std::true_type = fill / drain iteration (row predicates, special rows 0 and 1)
     auto body = [&](auto edge_tag) {
         constexpr bool EDGE = decltype(edge_tag)::value;
-#ifndef BTE_NO_WAIT_ST
         tm_wait_st();                                   // the partial sums stored in the previous iterations are in place
-#endif
         // E(t_v) dt/2 of the NV half-step times: broadcast reads, issued here so that the prefetch code below covers
         // their latency (volatile: kept out of the loop-invariant registers)
         double Ev[NV];
