@@ -15,14 +15,21 @@
 //   and runs the NS stages one after the other, all in registers: stage j takes the phi_y-difference D of row
 //   rho - j + 1 of X^j (its own K columns; the two outer neighbours by warp shuffle), which FINISHES row rho - j of
 //   X^{j+1} (started two iterations ago) and, with the own pairs X^{j-1}[rho - j + 2] that stage j - 2 has formed in
-//   this very iteration, STARTS row rho - j + 2 (cn_complete / cn_partial, bte_device.cuh).  The only state carried
-//   between iterations is the partial right-hand side (Pg, Ph) of the two rows in flight per stage and column;
+//   this very iteration, STARTS row rho - j + 2 (cn_apply / cn_partial, bte_device.cuh).  The only state carried
+//   between iterations is the partial right-hand side (Pg, Ph) of the two rows in flight per stage and column: it
+//   lives in TENSOR MEMORY (tcgen05.alloc once per CTA; tcgen05.st.x2 per value, tcgen05.ld.x16 per stage: a per-warp
+//   scratchpad of 2 NS slots, 6 x the shared-memory bandwidth on a path of its own), which frees 16 K registers per
+//   stage pair and is what makes K = 3 columns per lane fit;
 // * no barrier, no flag, no fence anywhere in the march: warps never exchange data.  The first / last HALO = NS - 1
 //   columns of a strip are recomputed halos (W = 32 K - 2 HALO owned columns); segments that cut a column at an
-//   arbitrary row recompute HALO halo rows on each side (trapezoid in n as in m);
-// * HBM -> shared memory: lane 0 issues two 1-D bulk copies per record (TMA engine, SASS UBLKCP) DPRE records ahead
-//   into a per-warp ring, completion on the slot's mbarrier; zero rows / columns outside the lattice are never read
-//   (boundary conditions (22)-(23)).  Results go to HBM straight from registers (128-bit stores);
+//   arbitrary row recompute HALO halo rows on each side (trapezoid in n as in m) with the UNPREDICATED loop body (what
+//   a stage forms outside its range is used by nobody; only the stores are limited to the segment's rows); predicated
+//   iterations remain at rows 0, 1 and beyond N of the lattice;
+// * HBM -> shared memory: one elected lane issues two 1-D bulk copies per record (TMA engine, SASS UBLKCP) DPRE records
+//   ahead into a per-warp ring, completion on the slot's mbarrier; zero rows / columns outside the lattice are never read
+//   (boundary conditions (22)-(23)).  The record of iteration rho + 1 is taken into registers at the END of iteration
+//   rho (its ring reads hide behind the loop edge).  Results go to HBM straight from registers (128-bit stores).  With
+//   EB = 8 the rows in HBM are fp32 pairs (bte_grid.precision 1): widened at the ring read, rounded once at the store;
 // * mu^t_{n,m} = n beta^t_m dt/2 (eq. 28-29) is formed as fma(n, B phi_m dt/2, n E(t) dt/2): the column part is two
 //   registers per column, the field part one number per row and half-step time (E(t_v) dt/2 sits in shared memory,
 //   read as a broadcast), so that no per-column table of the NS + 2 half-step times is needed -- registers are for
