@@ -384,7 +384,7 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
 #pragma unroll
         for (int v = 0; v < NV; ++v) Ev[v] = *(volatile double*)(&tabp[v]);
         unsigned Praw[SL];
-        tm_ld(tmS, Praw);                            // stage 0's rows in flight
+        if (!EDGE) tm_ld(tmS, Praw);                    // stage 0's rows in flight
         // ---- record rho: taken at the end of the previous iteration (its ring reads are hidden behind the loop edge) ----
         double2 Z[NS + 2][K];                           // Z[j + 2] = output of stage j; Z[0] = A, Z[1] = B
 #pragma unroll
@@ -402,8 +402,7 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
         // coefficients: they depend on (row, column, time) only, so the reciprocal chains are independent of each other
         // and of the data; they are formed for CG stages at a time (CG K independent chains side by side)
         bool landed = false;
-        form_mu(0);
-        form_mu(1);
+        if (!EDGE) { form_mu(0); form_mu(1); }
         double2 pq[NS][K];                              // (nu, mu') / (nu^2 + mu'^2) of stage j
         auto form_coef = [&](const int j0) {
 #pragma unroll
@@ -413,7 +412,7 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
 #pragma unroll
                 for (int q = 0; q < K; ++q) pq[j][q] = cn_coef(mu[j + 2][q], L.nu, L.nu2);
         };
-        form_coef(0);
+        if (!EDGE) form_coef(0);
 #pragma unroll
         for (int j = 0; j < NS; ++j) {
             // src = Z[j + 1] = row n + 1 of the stencil grid X^j, ownp = Z[j] = own pairs of row n + 2;
@@ -429,13 +428,27 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
                 comp = n >= lo && n <= hi;
                 strt = n + 2 >= lo && n + 2 <= hi;
             }
+            if (EDGE) {
+                // fill / drain and the ends of the lattice: a stage with neither a row to finish nor one to start costs
+                // nothing (its output reads as zero); an active one fetches its own rows in flight and coefficients
+                if (!(comp || strt)) {
+#pragma unroll
+                    for (int q = 0; q < K; ++q) Zo[q] = zero;
+                    continue;
+                }
+                tm_ld(tmS + (unsigned)(j * 2 * SL), Praw);
+                form_mu(j);
+                form_mu(j + 2);
+#pragma unroll
+                for (int q = 0; q < K; ++q) pq[j][q] = cn_coef(mu[j + 2][q], L.nu, L.nu2);
+            }
             // phi_y-difference of row n + 1 of the stencil grid: interior columns from registers, the two outer ones
             // from the adjacent lanes (stage 0: from the ring)
             double2 Lv, Rv;
             if (j == 0) { Lv = FL; Rv = FR; }
             else { Lv = shfl_up_d2(src[K - 1]); Rv = shfl_down_d2(src[0]); }
-            if ((j + 1) % Cfg::CG == 0 && j + 1 < NS) form_coef(j + 1);   // while the shuffles are in flight
-            // this stage's rows in flight have arrived; ask for the next stage's
+            if (!EDGE && (j + 1) % Cfg::CG == 0 && j + 1 < NS) form_coef(j + 1);   // while the shuffles are in flight
+            // this stage's rows in flight have arrived; (steady state) ask for the next stage's
             tm_wait_ld(Praw);
             double2 Pq[K];
 #pragma unroll
@@ -443,7 +456,7 @@ __device__ __forceinline__ void warpsweep_segment(const Layout& L, const int sys
                 Pq[q].x = __hiloint2double((int)Praw[4 * q + 1], (int)Praw[4 * q]);
                 Pq[q].y = __hiloint2double((int)Praw[4 * q + 3], (int)Praw[4 * q + 2]);
             }
-            if (j + 1 < NS) tm_ld(tmS + (unsigned)((j + 1) * 2 * SL), Praw);
+            if (!EDGE && j + 1 < NS) tm_ld(tmS + (unsigned)((j + 1) * 2 * SL), Praw);
             double2 D[K];
 #pragma unroll
             for (int q = 0; q < K; ++q) {
