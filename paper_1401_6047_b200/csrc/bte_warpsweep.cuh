@@ -234,9 +234,9 @@ __device__ __forceinline__ bool elect_one() {
     asm volatile("{\n .reg .pred p;\n elect.sync _|p, 0xffffffff;\n selp.u32 %0, 1, 0, p;\n}\n" : "=r"(ok));
     return ok != 0;
 }
-// a value every lane holds anyway, re-broadcast from lane 0 so that the compiler KNOWS it is warp-uniform and keeps it
-// (and everything derived from it) in uniform registers: the bulk-copy operands must be uniform, and the vector
-// registers are needed for the partial right-hand sides
+// a value every lane holds anyway, re-broadcast from lane 0: warp-uniform by construction whatever the compiler can
+// prove about threadIdx (the operands of the bulk copies and of the tensor-memory accesses must be uniform; ptxas still
+// keeps them in vector registers and converts with R2UR at the point of use)
 __device__ __forceinline__ int uni(int v) { return __shfl_sync(0xffffffffu, v, 0); }
 __device__ __forceinline__ unsigned uni(unsigned v) { return __shfl_sync(0xffffffffu, v, 0); }
 
