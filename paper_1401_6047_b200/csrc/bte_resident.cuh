@@ -219,22 +219,20 @@ __global__ void __launch_bounds__(1024, 1) resident_kernel(const __grid_constant
     }
     __syncthreads();
 
-    // this thread's points.  MODE 0 / 1: edge columns (jo = 0 and jo = Wv-1) first: e = tid, tid + T, ... < nE; then
-    // the interior columns 1 .. Wv-2: p = tid, tid + T, ... < rows * Wi, p = n * Wi + (jo - 1).
-    // MODE 2: all columns a group may ever update, jo = -el .. Wv + er - 1 (el, er = HB - 1 where a neighbour exists):
-    // p = n * Wi + (jo + el); a half-update skips the columns beyond its reach.
+    // this thread's points.  MODE 0 / 1: edge columns (jo = 0 and jo = Wv-1) first: e = T-1-tid, ... < nE (one point each,
+    // pushed to the neighbours), then the interior columns 1 .. Wv-2.  MODE 2: all columns a group may ever update,
+    // jo = -el .. Wv + er - 1 (el, er = HB - 1 where a neighbour exists); a half-update skips the columns beyond its reach.
+    // Interior / MODE 2: thread = (column j_first of Wi, row chunk n_first): rows [nA, nB) of that column, marched over n.
     const int el = (MODE == 2 && g > 0) ? HB - 1 : 0, er = (MODE == 2 && g < G - 1) ? HB - 1 : 0;
     const int nE = (MODE == 2) ? 0 : (Wv >= 2 ? 2 : 1) * rows;
     const int Wi = (MODE == 2) ? Wv + el + er : max(Wv - 2, 0), nI = rows * Wi;
     const int wi = max(Wi, 1);
     int n_first = tid / wi, j_first = tid - n_first * wi;
-    int dn = T / wi, dj = T - dn * wi;
-    // keep the quotients in registers: without this the compiler re-derives them (an integer division on the
-    // critical path of every half-update) to save four registers
-    asm volatile("" : "+r"(n_first), "+r"(j_first), "+r"(dn), "+r"(dj));
-    // MODE 2: thread = (column j_first, row chunk n_first): rows [nA, nB) of that column
     const int nch = max(T / wi, 1), Rr = (rows + nch - 1) / nch;
-    const int nA = (MODE == 2) ? min(n_first * Rr, rows) : 0, nB = (MODE == 2) ? min(nA + Rr, rows) : 0;
+    int nA = min(n_first * Rr, rows), nB = min(nA + Rr, rows);
+    // keep these in registers: without this the compiler re-derives them (integer divisions on the critical path of
+    // every half-update) to save registers
+    asm volatile("" : "+r"(n_first), "+r"(j_first), "+r"(nA), "+r"(nB));
     const unsigned sH = (unsigned)__cvta_generic_to_shared(Hs), sF = (unsigned)__cvta_generic_to_shared(Fs);
     const unsigned PB = (unsigned)P * 16;
     const unsigned sph = (unsigned)__cvta_generic_to_shared(phs), sgdt = (unsigned)__cvta_generic_to_shared(gdts),
@@ -287,12 +285,9 @@ __global__ void __launch_bounds__(1024, 1) resident_kernel(const __grid_constant
                             st_cluster_d2(cluster_map(sX + (unsigned)((n + 1) * P) * 16, g + 1), out);
                     }
                 }
-                int n = n_first, j = j_first;
-                for (int p = tid; p < nI; p += T) {
-                    resident_point(sX, sS, n, j + 2, PB, sph, sgdt, scn, c, L, Ea, Eb);
-                    j += dj; n += dn;
-                    if (j >= wi) { j -= wi; ++n; }
-                }
+                // interior columns 1 .. Wv-2: this thread's column segment, marching over n
+                if (nI > 0 && j_first < Wi && nA < nB)
+                    resident_column(sX, sS, nA, nB, j_first + 2, PB, sph, sgdt, scn, c, L, Ea, Eb);
             } else {
                 // half-update `sub` of the group: the slab and `reach` halo columns on each side (trapezoid in time)
                 const int reach = HB - 1 - sub;
