@@ -314,7 +314,7 @@ __global__ void __launch_bounds__(1024, 1) resident_kernel(const __grid_constant
                     for (int e = tid; e < 2 * HB * rows; e += T) {
                         const int cc = e / rows, nn = e - cc * rows;               // cc < HB: left edge, else right edge
                         const int jo = cc < HB ? cc : Wv - 2 * HB + cc;
-                        if (cc < HB || jo >= HB) resident_point(sX, sS, nn, jo + HB, PB, sph, sgdt, scn, c, L, Ea, Eb);
+                        if (cc < HB || jo >= HB) resident_column(sX, sS, nn, nn + 1, jo + HB, PB, sph, sgdt, scn, c, L, Ea, Eb);
                     }
                     asm volatile("bar.sync 1, %0;\n" ::"r"(T) : "memory");   // compute warps: the edge columns are done
                     const int per = HB * rows;                 // elements per (grid, side)
