@@ -151,4 +151,134 @@ __global__ void __launch_bounds__(128) rs_half_update_kernel(RsLayout L, int mod
     }
 }
 
+// ---- fast path: parallel cyclic reduction over phi_x (n_phix a power of two, <= RS_PCR_MAX_K) -----------------------------
+// The matrix of one phi_y column is CIRCULANT (sub-diagonal a = -gamma_b, diagonal b = nu, super-diagonal c = +gamma_b,
+// the same for every i), so parallel cyclic reduction needs the three numbers (a, b, c) per level and column only:
+//   level h = 1, 2, 4, .., K/2:   alpha = -a / b, beta = -c / b,
+//       d'_i = d_i + alpha d_{i-h} + beta d_{i+h}   (indices mod K),
+//       a' = alpha a,   b' = b + alpha c + beta a,   c' = beta c;
+//   after log2 K levels equation i couples x_i with x_{i +- K} = x_i:   x_i = d_i / (a + b + c).
+// b' = nu + 2 gamma^2 / nu after the first level and |a'| + |c'| < b' from then on: no pivoting needed.
+// A CTA of RS_PCR_WARPS warps takes a tile of RS_PCR_MT adjacent phi_y columns: all threads form the right-hand sides
+// of the tile in the coalesced (i, m) order of HBM (m fastest) into shared memory (transposed: one column contiguous),
+// then warp w reduces column w (lane l holds the elements i = l mod 32: conflict-free), and all threads store the tile
+// back in HBM order, folding norm and v_dr on the way.  HBM traffic: X read once and written once, the stencil grid
+// read once (+ the neighbour sector on either side of the tile): 24 B per point and half-update, no scratch arrays.
+constexpr int RS_PCR_MT = 8;
+constexpr int RS_PCR_WARPS = 8;
+constexpr int RS_PCR_T = 32 * RS_PCR_WARPS;
+constexpr int RS_PCR_MAX_K = 1024;
+static_assert(RS_PCR_MT == RS_PCR_WARPS && RS_PCR_T % RS_PCR_MT == 0, "one warp per column of the tile");
+
+__host__ __device__ inline int rs_pcr_pitch(int K) { return K + 4; }       // column pitch in shared memory: (K + 4) mod 16 = 4
+__host__ __device__ inline size_t rs_pcr_smem(int K) { return (size_t)2 * RS_PCR_MT * rs_pcr_pitch(K) * sizeof(double); }
+
+__global__ void __launch_bounds__(RS_PCR_T) rs_pcr_half_update_kernel(RsLayout L, int mode, long long k, int do_avg) {
+    extern __shared__ double rs_sm[];
+    __shared__ double red[2][RS_PCR_WARPS];
+    __shared__ unsigned int s_last;
+    const int K = L.K, P = rs_pcr_pitch(K), tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    double* bufA = rs_sm;
+    double* bufB = rs_sm + (size_t)RS_PCR_MT * P;
+    const size_t p = (size_t)L.pitch, G1 = (size_t)K * p;
+    double* X = (mode == 0) ? L.f : L.f + G1;
+    const double* S = (mode == 1) ? L.f : (mode == 0 ? L.f + G1 : L.f);
+    const double* Xs = (mode == 2) ? L.f : X;
+    const double delta = (mode == 2) ? 0.5 * L.dt : L.dt;
+    const double ta = (mode == 0) ? (double)k * L.dt : (mode == 1 ? ((double)k + 0.5) * L.dt : 0.0);
+    const double tb = (mode == 0) ? ((double)k + 1.0) * L.dt : (mode == 1 ? ((double)k + 1.5) * L.dt : 0.5 * L.dt);
+    const double nu = 1.0 + 0.5 * delta, xi = 1.0 - 0.5 * delta;
+    const int m0 = blockIdx.x * RS_PCR_MT;
+    const int ml = tid % RS_PCR_MT, m = m0 + ml;              // this thread's column in the load / store phases
+    const int i0 = tid / RS_PCR_MT;
+    constexpr int ISTEP = RS_PCR_T / RS_PCR_MT;
+    // 1. the tile of the source grid, transposed into bufA (pitch is a multiple of RS_PCR_MT: m < pitch always)
+    for (int i = i0; i < K; i += ISTEP) bufA[ml * P + i] = Xs[(size_t)i * p + m];
+    __syncthreads();
+    // 2. right-hand sides into bufB
+    {
+        const double ph = L.phi[m];
+        const double Ea = L.E_dc + L.E_omega * cos(L.omega * ta);
+        const double ga = (Ea + L.B * ph) * delta / (4.0 * L.dx);
+        const double kap = L.kappa_scale * L.B * delta / (2.0 * L.dphi);
+        const double gdt = L.gm[m] * delta;
+        const bool left = m > 0 && m < L.M1, right = m + 1 < L.M1;
+        const double* col = bufA + ml * P;
+        for (int i = i0; i < K; i += ISTEP) {
+            const double sl = left ? S[(size_t)i * p + m - 1] : 0.0, sr = right ? S[(size_t)i * p + m + 1] : 0.0;
+            const double xp1 = col[(i + 1) & (K - 1)], xm1 = col[(i - 1) & (K - 1)];
+            bufB[ml * P + i] = xi * col[i] - ga * (xp1 - xm1) + kap * L.sinx[i] * (sr - sl) + L.ex[i] * gdt;
+        }
+    }
+    __syncthreads();
+    // 3. warp w: parallel cyclic reduction of column m0 + w
+    double* src = bufB + warp * P;
+    double* dst = bufA + warp * P;
+    {
+        const double ph = L.phi[m0 + warp];
+        const double Eb = L.E_dc + L.E_omega * cos(L.omega * tb);
+        const double gb = (Eb + L.B * ph) * delta / (4.0 * L.dx);
+        double a = -gb, b = nu, c = gb;
+        for (int h = 1; h < K; h <<= 1) {
+            const double rb = 1.0 / b, alpha = -a * rb, beta = -c * rb;
+            const double a2 = alpha * a, b2 = b + alpha * c + beta * a, c2 = beta * c;
+            const double scale = (2 * h < K) ? 1.0 : 1.0 / (a2 + b2 + c2);      // last level: x_i = d_i / (a + b + c)
+            for (int i = lane; i < K; i += 32) {
+                const double v = src[i] + alpha * src[(i - h) & (K - 1)] + beta * src[(i + h) & (K - 1)];
+                dst[i] = v * scale;
+            }
+            __syncwarp();
+            a = a2; b = b2; c = c2;
+            double* t = src; src = dst; dst = t;
+        }
+    }
+    __syncthreads();
+    // 4. store (the result of every column sits in the same buffer: all columns run the same number of levels)
+    const double* res = (src == bufB + warp * P) ? bufB : bufA;
+    double sa = 0.0, sv = 0.0;
+    if (m < L.M1) {
+        for (int i = i0; i < K; i += ISTEP) {
+            const double x = res[ml * P + i];
+            X[(size_t)i * p + m] = x;
+            sa += x;
+            sv += L.sinx[i] * x;
+        }
+    }
+    if (mode != 0) return;
+    sa = rs_warp_sum(sa); sv = rs_warp_sum(sv);
+    if (lane == 0) { red[0][warp] = sa; red[1][warp] = sv; }
+    __syncthreads();
+    if (tid == 0) {
+        double qa = 0.0, qv = 0.0;
+        for (int w = 0; w < RS_PCR_WARPS; ++w) { qa += red[0][w]; qv += red[1][w]; }
+        L.partial[2 * blockIdx.x] = qa;
+        L.partial[2 * blockIdx.x + 1] = qv;
+        __threadfence();
+        s_last = (atomicAdd(&L.obs->done, 1u) + 1u == gridDim.x) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (s_last && warp == 0) {                                 // fixed-order fold: lane-strided sums, then the shuffle tree
+        __threadfence();
+        double qa = 0.0, qv = 0.0;
+        for (unsigned bq = lane; bq < gridDim.x; bq += 32) {
+            qa += __ldcg(L.partial + 2 * bq);
+            qv += __ldcg(L.partial + 2 * bq + 1);
+        }
+        qa = rs_warp_sum(qa); qv = rs_warp_sum(qv);
+        if (lane == 0) {
+            RsObs* o = L.obs;
+            o->norm = L.norm_scale * qa;
+            o->v_dr = L.norm_scale * qv;
+            if (do_avg) {
+                const double t = (double)(k + 1) * L.dt;
+                double sn, cs;
+                sincos(L.omega * t, &sn, &cs);
+                o->sum_v += o->v_dr * L.dt; o->sum_c += o->v_dr * cs * L.dt; o->sum_s += o->v_dr * sn * L.dt;
+                o->window += L.dt;
+            }
+            o->done = 0u;
+        }
+    }
+}
+
 }  // namespace bte

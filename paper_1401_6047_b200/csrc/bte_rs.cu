@@ -40,7 +40,7 @@ bool rs_grid_ok(const bte_rs_grid* g) {
 RsOffsets rs_offsets(const bte_rs_grid* g) {
     RsOffsets o{};
     o.pitch = (g->n_phiy + 7) / 8 * 8;
-    const size_t K = (size_t)g->n_phix, p = (size_t)o.pitch, blocks = (p + 127) / 128;
+    const size_t K = (size_t)g->n_phix, p = (size_t)o.pitch, blocks = p / RS_PCR_MT + 1;   // >= the blocks of either kernel
     size_t off = 0;
     o.f = off;       off = rs_align(off + 2 * K * p * sizeof(double));
     o.cprime = off;  off = rs_align(off + K * p * sizeof(double));
@@ -87,7 +87,23 @@ struct bte_rs_ctx {
     cudaStream_t stream;
     RsLayout L;
     int64_t k;          // whole-grid steps taken
+    bool pcr;           // n_phix a power of two <= RS_PCR_MAX_K: parallel cyclic reduction; else Thomas sweeps
 };
+
+namespace {
+
+// one half-update (mode as in bte_realspace.cuh) on the context's stream
+void rs_launch(bte_rs_ctx* c, int mode, long long k, int do_avg) {
+    if (c->pcr) {
+        const unsigned blocks = (unsigned)(c->off.pitch / RS_PCR_MT);
+        rs_pcr_half_update_kernel<<<blocks, RS_PCR_T, rs_pcr_smem(c->grid.n_phix), c->stream>>>(c->L, mode, k, do_avg);
+    } else {
+        const unsigned blocks = (unsigned)((c->off.pitch + 127) / 128);
+        rs_half_update_kernel<<<blocks, 128, 0, c->stream>>>(c->L, mode, k, do_avg);
+    }
+}
+
+}  // namespace
 
 extern "C" {
 
@@ -141,6 +157,12 @@ int bte_rs_create(const bte_rs_grid* grid, const bte_params* p, void* workspace,
     RS_CUDA_TRY(cudaStreamSynchronize(stream));
     bte_rs_ctx* c = new bte_rs_ctx();
     c->grid = *grid; c->params = *p; c->off = off; c->ws = ws; c->stream = stream; c->k = 0;
+    c->pcr = (K & (K - 1)) == 0 && K <= RS_PCR_MAX_K;
+    if (c->pcr) {
+        const cudaError_t e = cudaFuncSetAttribute(rs_pcr_half_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                   (int)rs_pcr_smem(RS_PCR_MAX_K));
+        if (e != cudaSuccess) { delete c; return rs_fail(BTE_ECUDA, "bte_rs_create: cudaFuncSetAttribute failed"); }
+    }
     RsLayout& L = c->L;
     L.K = K; L.M1 = M1; L.pitch = off.pitch; L.dt = grid->dt; L.dx = dx; L.dphi = dphi;
     L.E_dc = p->E_dc; L.E_omega = p->E_omega; L.omega = p->omega; L.B = p->B; L.kappa_scale = p->kappa_scale;
@@ -157,8 +179,7 @@ int bte_rs_init_equilibrium(bte_rs_ctx* c) {
     if (!c) return rs_fail(BTE_EINVAL, "bte_rs_init_equilibrium: NULL ctx");
     const dim3 g((unsigned)((c->off.pitch + 127) / 128), (unsigned)c->grid.n_phix);
     rs_init_kernel<<<g, 128, 0, c->stream>>>(c->L);
-    const unsigned blocks = (unsigned)((c->off.pitch + 127) / 128);
-    rs_half_update_kernel<<<blocks, 128, 0, c->stream>>>(c->L, 2, 0, 0);     // start-up z^{1/2}, L202
+    rs_launch(c, 2, 0, 0);                                                    // start-up z^{1/2}, L202
     RS_CUDA_TRY(cudaGetLastError());
     c->k = 0;
     return BTE_OK;
@@ -167,12 +188,11 @@ int bte_rs_init_equilibrium(bte_rs_ctx* c) {
 int bte_rs_step(bte_rs_ctx* c, int64_t n_steps) {
     if (!c) return rs_fail(BTE_EINVAL, "bte_rs_step: NULL ctx");
     if (n_steps < 0) return rs_fail(BTE_EINVAL, "bte_rs_step: n_steps < 0");
-    const unsigned blocks = (unsigned)((c->off.pitch + 127) / 128);
     for (int64_t s = 0; s < n_steps; ++s) {
         if (c->params.n_steps_total > 0 && c->k >= c->params.n_steps_total) break;   // frozen
         const int do_avg = (c->k + 1 > c->params.avg_start_step) ? 1 : 0;
-        rs_half_update_kernel<<<blocks, 128, 0, c->stream>>>(c->L, 0, (long long)c->k, do_avg);   // eq. (40)
-        rs_half_update_kernel<<<blocks, 128, 0, c->stream>>>(c->L, 1, (long long)c->k, 0);        // eq. (41), C5
+        rs_launch(c, 0, (long long)c->k, do_avg);      // eq. (40)
+        rs_launch(c, 1, (long long)c->k, 0);           // eq. (41), C5
         c->k += 1;
     }
     RS_CUDA_TRY(cudaGetLastError());

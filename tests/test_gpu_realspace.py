@@ -22,7 +22,7 @@ def run_pair(K, M1, n_steps, **kw):
     return s, sim, p, w.grid.dt
 
 
-@pytest.mark.parametrize("K,M1", [(4, 3), (16, 5), (37, 41), (64, 130), (128, 257)])
+@pytest.mark.parametrize("K,M1", [(4, 3), (8, 9), (16, 5), (37, 41), (64, 130), (96, 33), (128, 257), (512, 43), (1024, 19), (2048, 11)])
 def test_realspace_matches_oracle(K, M1):
     n_steps = 12 if K * M1 > 5000 else 30
     s, sim, p, dt = run_pair(K, M1, n_steps, dt=0.004, avg_start=3)
