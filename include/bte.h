@@ -172,7 +172,9 @@ BTE_API int bte_pendulum_averages(const bte_pendulum_params* params, int32_t n, 
  * One system per ctx; params as for bte_create (n_steps_total / avg_start_step honoured).  Same ownership rules:
  * caller-owned DEVICE workspace of bte_rs_workspace_bytes(grid) bytes, 256-byte aligned.  bte_rs_observables fills one
  * bte_obs (norm = sqrt(alpha) dx dphi sum f, eq. 6; v_dr = sqrt(alpha) dx dphi sum sin(phi_x) f, eq. 18-19; edge_leak 0).
- * bte_rs_get_state: f is a HOST array of n_phix * n_phiy doubles, [i][m], m fastest; grid_id 0 whole, 1 fractional. */
+ * bte_rs_get_state: f is a HOST array of n_phix * n_phiy doubles, [i][m], m fastest; grid_id 0 whole, 1 fractional.
+ * n_phix a power of two <= 1024 runs the parallel-cyclic-reduction kernel (one warp per phi_y column, in registers);
+ * any other n_phix the Thomas + Sherman-Morrison sweeps (one thread per phi_y point): same results to rounding. */
 typedef struct bte_rs_ctx bte_rs_ctx;
 typedef struct {
     int32_t n_phix;  /* periodic phi_x points, 4 .. 4096                                                   */

@@ -159,27 +159,34 @@ __global__ void __launch_bounds__(128) rs_half_update_kernel(RsLayout L, int mod
 //       a' = alpha a,   b' = b + alpha c + beta a,   c' = beta c;
 //   after log2 K levels equation i couples x_i with x_{i +- K} = x_i:   x_i = d_i / (a + b + c).
 // b' = nu + 2 gamma^2 / nu after the first level and |a'| + |c'| < b' from then on: no pivoting needed.
-// A CTA of RS_PCR_WARPS warps takes a tile of RS_PCR_MT adjacent phi_y columns: all threads form the right-hand sides
-// of the tile in the coalesced (i, m) order of HBM (m fastest) into shared memory (transposed: one column contiguous),
-// then warp w reduces column w (lane l holds the elements i = l mod 32: conflict-free), and all threads store the tile
-// back in HBM order, folding norm and v_dr on the way.  HBM traffic: X read once and written once, the stencil grid
-// read once (+ the neighbour sector on either side of the tile): 24 B per point and half-update, no scratch arrays.
+// A CTA of RS_PCR_MT warps takes a tile of RS_PCR_MT adjacent phi_y columns:
+//   1. all threads form the right-hand sides of the tile in the coalesced (i, m) order of HBM (m fastest) and put them
+//      into shared memory transposed (one column contiguous, column pitch K + 4: conflict-free both ways);
+//   2. warp w takes column w into REGISTERS, lane l the K / 32 elements i = l mod 32, and reduces it there: the levels
+//      h < 32 fetch d_{i -+ h} by warp shuffle (the source lane picks the register, r or r -+ 1, that the receiving lane's
+//      wrap-around needs), the levels h >= 32 are register-to-register; no barrier inside the reduction;
+//   3. all threads store the tile back in HBM order, folding norm and v_dr on the way.
+// HBM traffic: X read once and written once, the stencil grid read once (+ the neighbour sector on either side of
+// the tile): 24 B per point and half-update, no scratch arrays.
 constexpr int RS_PCR_MT = 8;
-constexpr int RS_PCR_WARPS = 8;
-constexpr int RS_PCR_T = 32 * RS_PCR_WARPS;
+constexpr int RS_PCR_T = 32 * RS_PCR_MT;
 constexpr int RS_PCR_MAX_K = 1024;
-static_assert(RS_PCR_MT == RS_PCR_WARPS && RS_PCR_T % RS_PCR_MT == 0, "one warp per column of the tile");
 
-__host__ __device__ inline int rs_pcr_pitch(int K) { return K + 4; }       // column pitch in shared memory: (K + 4) mod 16 = 4
-__host__ __device__ inline size_t rs_pcr_smem(int K) { return (size_t)2 * RS_PCR_MT * rs_pcr_pitch(K) * sizeof(double); }
+__host__ __device__ constexpr size_t rs_pcr_smem(int K) { return (size_t)RS_PCR_MT * (K + 4) * sizeof(double); }
 
-__global__ void __launch_bounds__(RS_PCR_T) rs_pcr_half_update_kernel(RsLayout L, int mode, long long k, int do_avg) {
+template <int K>
+__global__ void __launch_bounds__(RS_PCR_T, K >= 1024 ? 2 : K >= 512 ? 3 : 4) rs_pcr_half_update_kernel(RsLayout L, int mode, long long k, int do_avg) {
+    constexpr int R = K >= 32 ? K / 32 : 1;          // elements per lane
+    constexpr int LN = K >= 32 ? 32 : K;             // lanes that hold elements
+    constexpr int P = K + 4;                         // column pitch in shared memory: P mod 16 = 4 (K >= 16)
+    constexpr int MT = RS_PCR_MT;
+    constexpr int UNR = 4;                           // rows in flight per thread (5 loads each); 8 costs occupancy
+    constexpr int ISTEP = RS_PCR_T / MT;             // = 32 rows per sweep of the CTA
+    static_assert(ISTEP == 32 && (K & (K - 1)) == 0 && K >= 4, "tile shape");
     extern __shared__ double rs_sm[];
-    __shared__ double red[2][RS_PCR_WARPS];
+    __shared__ double red[2][MT];
     __shared__ unsigned int s_last;
-    const int K = L.K, P = rs_pcr_pitch(K), tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    double* bufA = rs_sm;
-    double* bufB = rs_sm + (size_t)RS_PCR_MT * P;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const size_t p = (size_t)L.pitch, G1 = (size_t)K * p;
     double* X = (mode == 0) ? L.f : L.f + G1;
     const double* S = (mode == 1) ? L.f : (mode == 0 ? L.f + G1 : L.f);
@@ -188,60 +195,92 @@ __global__ void __launch_bounds__(RS_PCR_T) rs_pcr_half_update_kernel(RsLayout L
     const double ta = (mode == 0) ? (double)k * L.dt : (mode == 1 ? ((double)k + 0.5) * L.dt : 0.0);
     const double tb = (mode == 0) ? ((double)k + 1.0) * L.dt : (mode == 1 ? ((double)k + 1.5) * L.dt : 0.5 * L.dt);
     const double nu = 1.0 + 0.5 * delta, xi = 1.0 - 0.5 * delta;
-    const int m0 = blockIdx.x * RS_PCR_MT;
-    const int ml = tid % RS_PCR_MT, m = m0 + ml;              // this thread's column in the load / store phases
-    const int i0 = tid / RS_PCR_MT;
-    constexpr int ISTEP = RS_PCR_T / RS_PCR_MT;
-    // 1. the tile of the source grid, transposed into bufA (pitch is a multiple of RS_PCR_MT: m < pitch always)
-    for (int i = i0; i < K; i += ISTEP) bufA[ml * P + i] = Xs[(size_t)i * p + m];
-    __syncthreads();
-    // 2. right-hand sides into bufB
+    const int m0 = blockIdx.x * MT;
+    const int ml = tid % MT, m = m0 + ml;            // this thread's column in the load / store phases (m < pitch)
+    const int i0 = tid / MT;                         // and its first row
+    // launched with programmatic stream serialization: the next half-update may become resident and form its constants
+    // now; it waits (griddepcontrol.wait) for THIS grid to complete and flush before it touches f or the observables
+    asm volatile("griddepcontrol.launch_dependents;");
+    // 1. right-hand sides, transposed into shared memory
     {
         const double ph = L.phi[m];
         const double Ea = L.E_dc + L.E_omega * cos(L.omega * ta);
         const double ga = (Ea + L.B * ph) * delta / (4.0 * L.dx);
         const double kap = L.kappa_scale * L.B * delta / (2.0 * L.dphi);
         const double gdt = L.gm[m] * delta;
+        asm volatile("griddepcontrol.wait;" ::: "memory");
         const bool left = m > 0 && m < L.M1, right = m + 1 < L.M1;
-        const double* col = bufA + ml * P;
-        for (int i = i0; i < K; i += ISTEP) {
-            const double sl = left ? S[(size_t)i * p + m - 1] : 0.0, sr = right ? S[(size_t)i * p + m + 1] : 0.0;
-            const double xp1 = col[(i + 1) & (K - 1)], xm1 = col[(i - 1) & (K - 1)];
-            bufB[ml * P + i] = xi * col[i] - ga * (xp1 - xm1) + kap * L.sinx[i] * (sr - sl) + L.ex[i] * gdt;
+        const double* Xc = Xs + m;
+        const double* Sc = S + m;
+#pragma unroll UNR
+        for (int j = 0; j < R; ++j) {
+            const int i = i0 + ISTEP * j;
+            if (K >= 32 || i < K) {
+                const double sl = left ? Sc[(size_t)i * p - 1] : 0.0, sr = right ? Sc[(size_t)i * p + 1] : 0.0;
+                const double xp1 = Xc[(size_t)((i + 1) & (K - 1)) * p], xm1 = Xc[(size_t)((i - 1) & (K - 1)) * p];
+                rs_sm[ml * P + i] = xi * Xc[(size_t)i * p] - ga * (xp1 - xm1) + kap * L.sinx[i] * (sr - sl) + L.ex[i] * gdt;
+            }
         }
     }
     __syncthreads();
-    // 3. warp w: parallel cyclic reduction of column m0 + w
-    double* src = bufB + warp * P;
-    double* dst = bufA + warp * P;
+    // 2. warp w: parallel cyclic reduction of column m0 + w in registers
     {
+        double* col = rs_sm + warp * P;
+        double d[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) d[r] = (K >= 32 || lane < K) ? col[lane + 32 * r] : 0.0;
         const double ph = L.phi[m0 + warp];
         const double Eb = L.E_dc + L.E_omega * cos(L.omega * tb);
         const double gb = (Eb + L.B * ph) * delta / (4.0 * L.dx);
         double a = -gb, b = nu, c = gb;
-        for (int h = 1; h < K; h <<= 1) {
+#pragma unroll
+        for (int h = 1; h < LN; h <<= 1) {                      // neighbours in other lanes
             const double rb = 1.0 / b, alpha = -a * rb, beta = -c * rb;
-            const double a2 = alpha * a, b2 = b + alpha * c + beta * a, c2 = beta * c;
-            const double scale = (2 * h < K) ? 1.0 : 1.0 / (a2 + b2 + c2);      // last level: x_i = d_i / (a + b + c)
-            for (int i = lane; i < K; i += 32) {
-                const double v = src[i] + alpha * src[(i - h) & (K - 1)] + beta * src[(i + h) & (K - 1)];
-                dst[i] = v * scale;
+            const bool wrap_up = lane >= LN - h, wrap_dn = lane < h;   // as a SOURCE: the receiver wrapped around the column
+            const int src_up = (lane - h) & (LN - 1), src_dn = (lane + h) & (LN - 1);
+            double dn[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const double send_up = wrap_up ? d[(r + R - 1) % R] : d[r];      // element i - h of the receiver
+                const double send_dn = wrap_dn ? d[(r + 1) % R] : d[r];          // element i + h of the receiver
+                const double up = __shfl_sync(0xffffffffu, send_up, src_up);
+                const double dw = __shfl_sync(0xffffffffu, send_dn, src_dn);
+                dn[r] = d[r] + alpha * up + beta * dw;
             }
-            __syncwarp();
+#pragma unroll
+            for (int r = 0; r < R; ++r) d[r] = dn[r];
+            const double a2 = alpha * a, b2 = b + alpha * c + beta * a, c2 = beta * c;
             a = a2; b = b2; c = c2;
-            double* t = src; src = dst; dst = t;
         }
+#pragma unroll
+        for (int q = 1; q < R; q <<= 1) {                       // h = 32 q: neighbours in this lane's own registers
+            const double rb = 1.0 / b, alpha = -a * rb, beta = -c * rb;
+            double dn[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) dn[r] = d[r] + alpha * d[(r + R - q) % R] + beta * d[(r + q) % R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) d[r] = dn[r];
+            const double a2 = alpha * a, b2 = b + alpha * c + beta * a, c2 = beta * c;
+            a = a2; b = b2; c = c2;
+        }
+        const double scale = 1.0 / (a + b + c);                 // x_i = d_i / (a + b + c)
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            if (K >= 32 || lane < K) col[lane + 32 * r] = d[r] * scale;
     }
     __syncthreads();
-    // 4. store (the result of every column sits in the same buffer: all columns run the same number of levels)
-    const double* res = (src == bufB + warp * P) ? bufB : bufA;
+    // 3. store in HBM order; norm (eq. 6) and v_dr (eq. 18-19) of a new whole grid
     double sa = 0.0, sv = 0.0;
     if (m < L.M1) {
-        for (int i = i0; i < K; i += ISTEP) {
-            const double x = res[ml * P + i];
-            X[(size_t)i * p + m] = x;
-            sa += x;
-            sv += L.sinx[i] * x;
+#pragma unroll 4
+        for (int j = 0; j < R; ++j) {
+            const int i = i0 + ISTEP * j;
+            if (K >= 32 || i < K) {
+                const double x = rs_sm[ml * P + i];
+                X[(size_t)i * p + m] = x;
+                sa += x;
+                sv += L.sinx[i] * x;
+            }
         }
     }
     if (mode != 0) return;
@@ -250,7 +289,7 @@ __global__ void __launch_bounds__(RS_PCR_T) rs_pcr_half_update_kernel(RsLayout L
     __syncthreads();
     if (tid == 0) {
         double qa = 0.0, qv = 0.0;
-        for (int w = 0; w < RS_PCR_WARPS; ++w) { qa += red[0][w]; qv += red[1][w]; }
+        for (int w = 0; w < MT; ++w) { qa += red[0][w]; qv += red[1][w]; }
         L.partial[2 * blockIdx.x] = qa;
         L.partial[2 * blockIdx.x + 1] = qv;
         __threadfence();
@@ -278,6 +317,22 @@ __global__ void __launch_bounds__(RS_PCR_T) rs_pcr_half_update_kernel(RsLayout L
             }
             o->done = 0u;
         }
+    }
+}
+
+using RsKernel = void (*)(RsLayout, int, long long, int);
+inline RsKernel rs_pcr_kernel_for(int K) {
+    switch (K) {
+        case 4: return rs_pcr_half_update_kernel<4>;
+        case 8: return rs_pcr_half_update_kernel<8>;
+        case 16: return rs_pcr_half_update_kernel<16>;
+        case 32: return rs_pcr_half_update_kernel<32>;
+        case 64: return rs_pcr_half_update_kernel<64>;
+        case 128: return rs_pcr_half_update_kernel<128>;
+        case 256: return rs_pcr_half_update_kernel<256>;
+        case 512: return rs_pcr_half_update_kernel<512>;
+        case 1024: return rs_pcr_half_update_kernel<1024>;
+        default: return nullptr;
     }
 }
 

@@ -87,7 +87,7 @@ struct bte_rs_ctx {
     cudaStream_t stream;
     RsLayout L;
     int64_t k;          // whole-grid steps taken
-    bool pcr;           // n_phix a power of two <= RS_PCR_MAX_K: parallel cyclic reduction; else Thomas sweeps
+    RsKernel pcr;       // n_phix a power of two <= RS_PCR_MAX_K: parallel cyclic reduction; else NULL: Thomas sweeps
 };
 
 namespace {
@@ -96,7 +96,14 @@ namespace {
 void rs_launch(bte_rs_ctx* c, int mode, long long k, int do_avg) {
     if (c->pcr) {
         const unsigned blocks = (unsigned)(c->off.pitch / RS_PCR_MT);
-        rs_pcr_half_update_kernel<<<blocks, RS_PCR_T, rs_pcr_smem(c->grid.n_phix), c->stream>>>(c->L, mode, k, do_avg);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(blocks); cfg.blockDim = dim3(RS_PCR_T);
+        cfg.dynamicSmemBytes = rs_pcr_smem(c->grid.n_phix); cfg.stream = c->stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;    // prologue of this launch overlaps the previous one
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        cudaLaunchKernelEx(&cfg, c->pcr, c->L, mode, k, do_avg);
     } else {
         const unsigned blocks = (unsigned)((c->off.pitch + 127) / 128);
         rs_half_update_kernel<<<blocks, 128, 0, c->stream>>>(c->L, mode, k, do_avg);
@@ -157,10 +164,9 @@ int bte_rs_create(const bte_rs_grid* grid, const bte_params* p, void* workspace,
     RS_CUDA_TRY(cudaStreamSynchronize(stream));
     bte_rs_ctx* c = new bte_rs_ctx();
     c->grid = *grid; c->params = *p; c->off = off; c->ws = ws; c->stream = stream; c->k = 0;
-    c->pcr = (K & (K - 1)) == 0 && K <= RS_PCR_MAX_K;
+    c->pcr = rs_pcr_kernel_for(K);
     if (c->pcr) {
-        const cudaError_t e = cudaFuncSetAttribute(rs_pcr_half_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                   (int)rs_pcr_smem(RS_PCR_MAX_K));
+        const cudaError_t e = cudaFuncSetAttribute(c->pcr, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rs_pcr_smem(K));
         if (e != cudaSuccess) { delete c; return rs_fail(BTE_ECUDA, "bte_rs_create: cudaFuncSetAttribute failed"); }
     }
     RsLayout& L = c->L;
