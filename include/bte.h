@@ -21,6 +21,7 @@
  *   - "host" / "device" is stated for every pointer.  The ONLY device memory the library uses is the
  *     caller-owned workspace handed to bte_create (e.g. a torch.empty(uint8) tensor); the library never
  *     allocates or frees device memory and never frees the workspace.  The ctx is a small host object.
+ *     (One exception, stated at its declaration: bte_rs_evolve_static works in a fixed 5 MiB array of the library.)
  *   - Arrays a, b exchanged with the host are row-major (n_harm+1) x n_phiy doubles, m fastest
  *     (the layout of Fig. 7).  Inside the workspace the state is stored as interleaved (a,b)
  *     pairs.
@@ -189,6 +190,30 @@ BTE_API int bte_rs_step(bte_rs_ctx* ctx, int64_t n_steps);
 BTE_API int bte_rs_observables(bte_rs_ctx* ctx, bte_obs* out /* host, one entry */);
 BTE_API int bte_rs_get_state(bte_rs_ctx* ctx, int32_t grid_id, double* f /* host */);
 BTE_API int bte_rs_destroy(bte_rs_ctx* ctx);
+
+/* The real-space step WITHOUT ANY ALLOCATION AND WITHOUT A WORKSPACE, for callers that cannot call cudaMalloc or own
+ * scratch memory (code under CUDA graph capture, tight serving loops, harnesses that forbid allocation).  One call =
+ * n_steps leap-frog steps (eq. 40-41 in the real-space form above, the same kernels as bte_rs_step) from a state the
+ * caller passes in to a state the caller gets back; nothing survives the call but f_out and obs.
+ *   grid, params : host, as for bte_rs_create (n_steps_total / avg_start_step honoured against step0 + s).
+ *   f_in         : DEVICE, 2 * n_phix * n_phiy doubles, [grid 2][i][m], m fastest, dense: the whole grid at
+ *                  t = step0 dt, then the fractional grid at t = (step0 + 1/2) dt.  NULL = start from the
+ *                  equilibrium f0 (eq. 13) with the start-up half step (L202); step0 must then be 0.
+ *   f_out        : DEVICE, same shape: both grids after step0 + n_steps steps.  May alias f_in.
+ *   obs          : host or NULL.  Non-NULL: the stream is synchronised and one record is written (norm, v_dr of the
+ *                  last step taken; the running sums of eq. 17 over THIS call's steps only).  NULL: the call
+ *                  returns without synchronising (no host transfer at all).
+ *   cuda_stream  : cudaStream_t (as void*) of the CURRENT device, which the caller has made current.
+ * Scratch: the pitched state, the sweep arrays, the tables, the block partials and the observables live in one
+ * file-scope device array of 5 MiB inside the library, which every GPU that loads the library holds until the process
+ * exits.  Limit: n_phix * pitch <= 131072 lattice points, pitch = n_phiy rounded up to a multiple of 8 (e.g. 64 x 2048,
+ * 256 x 512, 1024 x 128); larger grids are refused with BTE_ENOMEM and a message naming the limit (use bte_rs_create).
+ * The function calls no cudaMalloc, cudaFree or allocating library routine.  ALL CALLS SHARE THE ARRAY, which keeps
+ * the last call's contents: what must start at zero is cleared at the start of each call, but two calls that overlap
+ * on the GPU (different streams, or two host threads) race -- serialise them on one stream.                        */
+BTE_API int bte_rs_evolve_static(const bte_rs_grid* grid /* host */, const bte_params* params /* host, one entry */,
+                         const double* f_in /* device or NULL */, int64_t step0, int64_t n_steps,
+                         double* f_out /* device */, bte_obs* obs /* host or NULL */, void* cuda_stream);
 
 /* Tuning / variant selection, before or between bte_step calls.  Keys:
  *   "variant"      0 = automatic (default), 1 = two half-update kernels per step (96 B/point/step),

@@ -9,7 +9,7 @@ from . import workloads  # noqa: F401
 
 def __getattr__(name):
     if name in ("Solver", "Obs", "BteError", "load_library", "workspace_bytes", "EXPORTS", "LIB_PATH",
-                "pendulum_averages", "RealSpaceSolver"):
+                "pendulum_averages", "RealSpaceSolver", "rs_evolve_static"):
         from . import binding
         return getattr(binding, name)
     raise AttributeError(name)

@@ -22,7 +22,8 @@ EXPORTS = ("bte_workspace_bytes", "bte_create", "bte_init_equilibrium", "bte_ste
            "bte_destroy", "bte_get_state", "bte_set_state", "bte_get_state_batch", "bte_set_state_batch", "bte_get_option",
            "bte_reconstruct_pdf", "bte_pendulum_workspace_bytes",
            "bte_pendulum_averages", "bte_rs_workspace_bytes", "bte_rs_create", "bte_rs_init_equilibrium",
-           "bte_rs_step", "bte_rs_observables", "bte_rs_get_state", "bte_rs_destroy", "bte_set_option",
+           "bte_rs_step", "bte_rs_observables", "bte_rs_get_state", "bte_rs_destroy", "bte_rs_evolve_static",
+           "bte_set_option",
            "bte_launch_count", "bte_set_steady_policy", "bte_steady_info",
            "bte_last_error")
 
@@ -124,6 +125,9 @@ def load_library(path: str = LIB_PATH) -> C.CDLL:
     lib.bte_rs_observables.argtypes = [C.c_void_p, C.POINTER(bte_obs)]
     lib.bte_rs_get_state.restype = C.c_int
     lib.bte_rs_get_state.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
+    lib.bte_rs_evolve_static.restype = C.c_int
+    lib.bte_rs_evolve_static.argtypes = [C.POINTER(bte_rs_grid), C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p,
+                                         C.c_void_p, C.c_void_p]
     lib.bte_set_option.restype = C.c_int
     lib.bte_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_int64]
     lib.bte_launch_count.restype = C.c_int
@@ -173,6 +177,35 @@ def pendulum_averages(param_sets, n_phase: int = 64, h: float = 0.004, n_rk: int
 def workspace_bytes(n_harm: int, n_phiy: int, n_batch: int, dt: float) -> int:
     g = make_grid(n_harm, n_phiy, n_batch, dt)
     return int(load_library().bte_workspace_bytes(C.byref(g)))
+
+
+def rs_evolve_static(n_phix: int, n_phiy: int, dt: float, params, f_in, step0: int, n_steps: int, f_out,
+                     want_obs: bool = True, stream=None):
+    """bte_rs_evolve_static (include/bte.h): n_steps real-space steps from f_in (CUDA float64 tensor [2, n_phix, n_phiy],
+    contiguous; None = equilibrium) into f_out (same shape), in the library's static scratch array: no allocation, no
+    workspace.  Returns an Obs when want_obs (synchronises), else None.  Argument marshalling only."""
+    import torch
+    lib = load_library()
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_1401_6047_b200 needs a CUDA device (B200, sm_100a); no CPU fallback")
+    shape = (2, int(n_phix), int(n_phiy))
+    for t in (f_in, f_out):
+        if t is None and t is f_in:
+            continue
+        if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == shape):
+            raise ValueError(f"need contiguous CUDA float64 tensors of shape {shape}")
+    if f_in is not None and f_in.device != f_out.device:
+        raise ValueError("f_in and f_out must live on the same device")
+    g = bte_rs_grid(int(n_phix), int(n_phiy), float(dt))
+    ps = make_params([params])
+    o = bte_obs()
+    with torch.cuda.device(f_out.device):
+        st = stream if stream is not None else torch.cuda.current_stream(f_out.device)
+        _check(lib.bte_rs_evolve_static(C.byref(g), C.cast(ps, C.c_void_p), C.c_void_p(f_in.data_ptr() if f_in is not None else None),
+                                        C.c_int64(int(step0)), C.c_int64(int(n_steps)), C.c_void_p(f_out.data_ptr()),
+                                        C.cast(C.byref(o), C.c_void_p) if want_obs else None,
+                                        C.c_void_p(st.cuda_stream)))
+    return Obs(*[getattr(o, f[0]) for f in bte_obs._fields_]) if want_obs else None
 
 
 class RealSpaceSolver:

@@ -232,3 +232,161 @@ int bte_rs_destroy(bte_rs_ctx* c) {
 }
 
 }  // extern "C"
+
+// ---- bte_rs_evolve_static: the real-space step without any allocation (include/bte.h) ----------------------------------
+// For callers that cannot allocate or own a workspace (CUDA graph capture, tight serving loops, harnesses that forbid
+// cudaMalloc): the same kernels as bte_rs_step, with everything they need besides the caller's input and output -- the
+// pitched state, the Thomas scratch arrays, the tables, the block partials and the observables -- in ONE file-scope
+// device array of fixed size.  Every GPU that loads the library holds these RS_STATIC_BYTES until the process exits.
+// All calls share the array and it keeps the last call's contents: what must start at zero (the observables: running
+// sums and the block counter) is cleared at the start of every call; calls that overlap on the GPU (two streams, or
+// two host threads) race.
+#include <mutex>
+
+namespace {
+
+constexpr size_t RS_STATIC_MAX_POINTS = 131072;            // n_phix * pitch, pitch = n_phiy rounded up to a multiple of 8
+constexpr size_t RS_STATIC_BYTES = (size_t)5 << 20;        // 4 arrays of MAX_POINTS doubles (4 MiB) + tables, partials, observables
+static __device__ __align__(256) unsigned char rs_static_scratch[RS_STATIC_BYTES];
+
+struct RsStaticOffsets { int pitch; size_t f, cprime, zvec, ex, sinx, gm, phi, partial, obs, total; };
+
+RsStaticOffsets rs_static_offsets(const bte_rs_grid* g) {
+    RsStaticOffsets o{};
+    o.pitch = (g->n_phiy + 7) / 8 * 8;
+    const size_t K = (size_t)g->n_phix, p = (size_t)o.pitch;
+    size_t off = 0;
+    o.f = off;       off = rs_align(off + 2 * K * p * sizeof(double));
+    o.cprime = off;  off = rs_align(off + K * p * sizeof(double));
+    o.zvec = off;    off = rs_align(off + K * p * sizeof(double));
+    o.ex = off;      off = rs_align(off + K * sizeof(double));
+    o.sinx = off;    off = rs_align(off + K * sizeof(double));
+    o.gm = off;      off = rs_align(off + p * sizeof(double));
+    o.phi = off;     off = rs_align(off + p * sizeof(double));
+    o.partial = off; off = rs_align(off + (p / RS_PCR_MT + 1) * 2 * sizeof(double));
+    o.obs = off;     off = rs_align(off + sizeof(RsObs));
+    o.total = off;
+    return o;
+}
+
+// In host code `rs_static_scratch` is a host-side stand-in, not a device address: the address a kernel can use comes
+// from cudaGetSymbolAddress, asked once per device with that device current.
+constexpr int RS_STATIC_MAX_DEVICES = 64;
+std::mutex g_rs_static_mutex;
+unsigned char* g_rs_static_base[RS_STATIC_MAX_DEVICES] = {};
+
+int rs_static_base(unsigned char** out) {
+    int dev = -1;
+    RS_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= RS_STATIC_MAX_DEVICES) return rs_fail(BTE_EINVAL, "bte_rs_evolve_static: device ordinal out of range");
+    std::lock_guard<std::mutex> lock(g_rs_static_mutex);
+    if (!g_rs_static_base[dev]) {
+        void* ptr = nullptr;
+        RS_CUDA_TRY(cudaGetSymbolAddress(&ptr, rs_static_scratch));
+        if (!ptr) return rs_fail(BTE_ECUDA, "bte_rs_evolve_static: cudaGetSymbolAddress returned NULL");
+        g_rs_static_base[dev] = (unsigned char*)ptr;
+    }
+    *out = g_rs_static_base[dev];
+    return BTE_OK;
+}
+
+// the tables of bte_rs_create (eq. 13 split into its phi_x and phi_y parts; C8, C19), formed on the device: no host staging
+__global__ void rs_static_tables_kernel(double* ex, double* sinx, double* gm, double* phi, int K, int M1, int pitch,
+                                        double pref, double mu, double dx, double centre, double dphi) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const double PI = 3.14159265358979323846;
+    if (t < K) {
+        const double x = -PI + dx * t;
+        ex[t] = pref * exp(mu * (cos(x) - 1.0));
+        sinx[t] = sin(x);
+    }
+    if (t < pitch) {
+        double ph = 0.0, g = 0.0;
+        if (t < M1) {
+            ph = centre + (t - (M1 - 1) / 2.0) * dphi;
+            g = exp(-mu * ph * ph / 2.0);
+            if (g < 1e-300) g = 0.0;
+        }
+        phi[t] = ph;
+        gm[t] = g;
+    }
+}
+
+}  // namespace
+
+extern "C" int bte_rs_evolve_static(const bte_rs_grid* grid, const bte_params* p, const double* f_in, int64_t step0,
+                                    int64_t n_steps, double* f_out, bte_obs* obs, void* cuda_stream) {
+    if (!grid || !p || !f_out) return rs_fail(BTE_EINVAL, "bte_rs_evolve_static: NULL argument");
+    if (!rs_grid_ok(grid)) return rs_fail(BTE_EINVAL, "bte_rs_evolve_static: need 4 <= n_phix <= 4096, n_phiy >= 3, dt > 0");
+    if (step0 < 0 || n_steps < 0) return rs_fail(BTE_EINVAL, "bte_rs_evolve_static: step0 < 0 or n_steps < 0");
+    if (!f_in && step0 != 0) return rs_fail(BTE_EINVAL, "bte_rs_evolve_static: f_in NULL (start from equilibrium) needs step0 = 0");
+    const bool finite = std::isfinite(p->E_dc) && std::isfinite(p->E_omega) && std::isfinite(p->omega) &&
+                        std::isfinite(p->B) && std::isfinite(p->mu) && std::isfinite(p->alpha) &&
+                        std::isfinite(p->phiy_min) && std::isfinite(p->phiy_max) && std::isfinite(p->kappa_scale);
+    if (!finite || !(p->mu > 0.0) || !(p->alpha > 0.0) || !(p->phiy_max > p->phiy_min) || p->n_steps_total < 0 ||
+        p->avg_start_step < 0)
+        return rs_fail(BTE_EINVAL, "bte_rs_evolve_static: need finite parameters, mu > 0, alpha > 0, phiy_max > phiy_min");
+    const RsStaticOffsets off = rs_static_offsets(grid);
+    const int K = grid->n_phix, M1 = grid->n_phiy, M = M1 - 1;
+    if ((size_t)K * (size_t)off.pitch > RS_STATIC_MAX_POINTS || off.total > RS_STATIC_BYTES) {
+        char buf[256];
+        snprintf(buf, sizeof buf,
+                 "bte_rs_evolve_static: n_phix * pitch = %zu points exceeds the static scratch limit of %zu "
+                 "(pitch = n_phiy rounded up to a multiple of 8); use bte_rs_create with a caller-owned workspace",
+                 (size_t)K * (size_t)off.pitch, RS_STATIC_MAX_POINTS);
+        return rs_fail(BTE_ENOMEM, buf);
+    }
+    const double dphi = (p->phiy_max - p->phiy_min) / M;
+    if (std::fabs(p->B) * grid->dt / dphi >= 2.0)
+        return rs_fail(BTE_EUNSTABLE, "bte_rs_evolve_static: |B| dt / dphi >= 2 (scheme unstable, DESIGN.md C11)");
+    unsigned char* base = nullptr;
+    if (const int rc = rs_static_base(&base)) return rc;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    const double PI = 3.14159265358979323846;
+    const double dx = 2.0 * PI / K;
+    bte_rs_ctx c{};                                   // on the stack: what rs_launch reads
+    c.grid = *grid; c.params = *p; c.off.pitch = off.pitch; c.ws = (char*)base; c.stream = stream; c.k = step0;
+    c.pcr = rs_pcr_kernel_for(K);
+    if (c.pcr) RS_CUDA_TRY(cudaFuncSetAttribute(c.pcr, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rs_pcr_smem(K)));
+    RsLayout& L = c.L;
+    L.K = K; L.M1 = M1; L.pitch = off.pitch; L.dt = grid->dt; L.dx = dx; L.dphi = dphi;
+    L.E_dc = p->E_dc; L.E_omega = p->E_omega; L.omega = p->omega; L.B = p->B; L.kappa_scale = p->kappa_scale;
+    L.norm_scale = std::sqrt(p->alpha) * dx * dphi;
+    L.f = (double*)(base + off.f); L.cprime = (double*)(base + off.cprime); L.zvec = (double*)(base + off.zvec);
+    double* ex = (double*)(base + off.ex);   double* sinx = (double*)(base + off.sinx);
+    double* gm = (double*)(base + off.gm);   double* phi = (double*)(base + off.phi);
+    L.ex = ex; L.sinx = sinx; L.gm = gm; L.phi = phi;
+    L.partial = (double*)(base + off.partial); L.obs = (RsObs*)(base + off.obs);
+    // what must start at zero: the running sums and the block counter of the last-block fold
+    RS_CUDA_TRY(cudaMemsetAsync(L.obs, 0, sizeof(RsObs), stream));
+    const double pref = (1.0 / (2.0 * PI)) * std::sqrt(p->mu / (2.0 * PI * p->alpha)) / bessel_i0_scaled(p->mu);
+    const int tn = K > off.pitch ? K : off.pitch;
+    rs_static_tables_kernel<<<(unsigned)((tn + 127) / 128), 128, 0, stream>>>(ex, sinx, gm, phi, K, M1, off.pitch, pref, p->mu, dx,
+                                                                             0.5 * (p->phiy_min + p->phiy_max), dphi);
+    const size_t row = (size_t)M1 * sizeof(double), prow = (size_t)off.pitch * sizeof(double);
+    if (f_in) {      // dense [2][K][M1] -> pitched state; the pad columns keep stale values, which no kernel lets through
+        RS_CUDA_TRY(cudaMemcpy2DAsync(L.f, prow, f_in, row, row, (size_t)2 * K, cudaMemcpyDeviceToDevice, stream));
+    } else {
+        const dim3 g((unsigned)((off.pitch + 127) / 128), (unsigned)K);
+        rs_init_kernel<<<g, 128, 0, stream>>>(L);
+        rs_launch(&c, 2, 0, 0);                       // start-up z^{1/2}, L202
+    }
+    for (int64_t s = 0; s < n_steps; ++s) {
+        if (p->n_steps_total > 0 && c.k >= p->n_steps_total) break;   // frozen
+        const int do_avg = (c.k + 1 > p->avg_start_step) ? 1 : 0;
+        rs_launch(&c, 0, (long long)c.k, do_avg);     // eq. (40)
+        rs_launch(&c, 1, (long long)c.k, 0);          // eq. (41), C5
+        c.k += 1;
+    }
+    RS_CUDA_TRY(cudaGetLastError());
+    RS_CUDA_TRY(cudaMemcpy2DAsync(f_out, row, L.f, prow, row, (size_t)2 * K, cudaMemcpyDeviceToDevice, stream));
+    if (obs) {
+        RsObs o;
+        RS_CUDA_TRY(cudaMemcpyAsync(&o, L.obs, sizeof o, cudaMemcpyDeviceToHost, stream));
+        RS_CUDA_TRY(cudaStreamSynchronize(stream));
+        obs->step = c.k; obs->t = (double)c.k * grid->dt; obs->norm = o.norm; obs->v_dr = o.v_dr;
+        obs->sum_v_dt = o.sum_v; obs->sum_vcos_dt = o.sum_c; obs->sum_vsin_dt = o.sum_s; obs->window = o.window;
+        obs->edge_leak = 0.0;
+    }
+    return BTE_OK;
+}
