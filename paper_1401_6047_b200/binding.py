@@ -233,20 +233,28 @@ class RealSpaceSolver:
                                      nbytes, C.c_void_p(self.stream.cuda_stream), C.byref(h)))
             self._h = h
 
+    def _on_device(self):
+        import torch
+        return torch.cuda.device(self.device)      # the bte_rs_* calls launch on the current device
+
     def init_equilibrium(self):
-        _check(self._lib.bte_rs_init_equilibrium(self._h))
+        with self._on_device():
+            _check(self._lib.bte_rs_init_equilibrium(self._h))
 
     def step(self, n_steps: int):
-        _check(self._lib.bte_rs_step(self._h, int(n_steps)))
+        with self._on_device():
+            _check(self._lib.bte_rs_step(self._h, int(n_steps)))
 
     def observables(self) -> "Obs":
         o = bte_obs()
-        _check(self._lib.bte_rs_observables(self._h, C.byref(o)))
+        with self._on_device():
+            _check(self._lib.bte_rs_observables(self._h, C.byref(o)))
         return Obs(*[getattr(o, f[0]) for f in bte_obs._fields_])
 
     def get_state(self, grid_id: int):
         f = np.empty(self.shape)
-        _check(self._lib.bte_rs_get_state(self._h, grid_id, C.c_void_p(f.ctypes.data)))
+        with self._on_device():
+            _check(self._lib.bte_rs_get_state(self._h, grid_id, C.c_void_p(f.ctypes.data)))
         return f
 
     def destroy(self):
