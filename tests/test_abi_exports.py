@@ -123,3 +123,26 @@ def test_product_does_not_import_the_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(from|import)\s+oracle\b", text, flags=re.M), f
                 assert "bte_oracle" not in text, f
+
+
+def test_rs_evolve_static_validates_before_any_cuda_call(lib):
+    """bte_rs_evolve_static: NULL arguments, bad step arguments and grids beyond the static scratch limit (131072 points)
+    are refused by host-side checks; the dummy device pointers below are never touched."""
+    from paper_1401_6047_b200 import binding, workloads as W
+    p = binding.make_params([W.small_case(N=2, M1=41, dt=0.004).params[0]])
+    dummy = C.c_void_p(0x10000)
+
+    def call(K, M1, f_in, step0, n_steps, f_out, params=p):
+        g = binding.bte_rs_grid(K, M1, 0.004)
+        return lib.bte_rs_evolve_static(C.byref(g), C.cast(params, C.c_void_p) if params is not None else None, f_in,
+                                        C.c_int64(step0), C.c_int64(n_steps), f_out, None, None)
+
+    assert call(64, 130, None, 0, 1, None) == -1                                   # no output
+    assert call(64, 130, None, 0, 1, dummy, params=None) == -1                     # no parameters
+    assert call(2, 130, None, 0, 1, dummy) == -1                                   # too few phi_x points
+    assert call(64, 130, None, 0, -1, dummy) == -1 and call(64, 130, dummy, -1, 1, dummy) == -1
+    assert call(64, 130, None, 5, 1, dummy) == -1                                  # equilibrium start needs step0 = 0
+    assert call(256, 520, None, 0, 1, dummy) == -3                                 # 256 x 520 > 131072 points
+    msg = lib.bte_last_error().decode()
+    assert "131072" in msg and "bte_rs_create" in msg
+    assert call(4096, 40, None, 0, 1, dummy) == -3                                 # 4096 x 40 = 163840 points
