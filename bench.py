@@ -381,10 +381,14 @@ def alu_roofline(updates_per_block, ms, steps, launches):
                            f"{FP64_PER_HALF_UPDATE} fp64 instructions per half-update"}
 
 
-def time_workload(cx, w, steps, warmup, min_blocks, sample_clocks, one_pass=False):
+def time_workload(cx, w, steps, warmup, min_blocks, sample_clocks, one_pass=False, precision=None):
     """Device-resident measurement of one workload: state already in HBM when the timed region starts."""
     from paper_1401_6047_b200 import Solver
+    import copy
     args = cx.args
+    if precision is not None and precision != args.precision:
+        args = copy.copy(args)
+        args.precision = precision
     peak, peak_src = measured_peak_gbs()
     s = Solver(w.grid, w.params, device=cx.dev, precision=args.precision)
     apply_options(s, args)
@@ -493,6 +497,14 @@ def run_ours(args):
             r["config"] = config_of(wi)
             configs[wi.name] = r
 
+    # NEXT-4 beside the headline, never as the headline: the same workload with the state stored as fp32 pairs (the
+    # paper's storage precision) and fp64 arithmetic, through the same production kernel
+    other_precisions = {}
+    if not args.no_other_configs and cx.world == 1 and args.precision == 0 and not args.sweep_steps and args.variant == 0:
+        r, _ = time_workload(cx, w, min(240, args.steps), 6, 3, False, precision=1)
+        r["dtype"] = "f32 storage / f64 arithmetic"
+        other_precisions["f32_storage"] = r
+
     if cx.rank != 0:
         if cx.dist.is_initialized():
             cx.dist.destroy_process_group()
@@ -518,7 +530,7 @@ def run_ours(args):
         "gpu_launches": main["gpu_launches"],
         "clocks": clocks,
         "check": dict(main["check"], e2e_step=e2e_step),
-        "configs": configs,
+        "configs": configs, "other_precisions": other_precisions,
     }
     if w.name == "paper_table1":
         # the paper's own workload and MLUPS convention (n-harmonics x g-grid x steps / time, L328); its number is

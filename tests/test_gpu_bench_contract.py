@@ -33,6 +33,9 @@ def test_default_workload_line():
     assert r["bound"] == "hbm" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
     assert r["kernel"] in ("sweep_kernel", "warpsweep_kernel") and 0.3 < r["frac"] < 1.1
     assert r["one_step_per_pass"]["launches"] == r["one_step_per_pass"]["steps"]
+    f32 = d["other_precisions"]["f32_storage"]        # NEXT-4 leg beside the headline: same kernel, fp32 pairs in HBM
+    assert f32["dtype"] == "f32 storage / f64 arithmetic" and f32["kernel"] == "warpsweep_kernel" and f32["value"] > 0
+    assert abs(f32["check"]["norm"] - 1.0) < 1e-4 and f32["steps"] == 60
     assert 0.5 < r["one_step_per_pass"]["frac"] < 1.1                         # the HBM-bound form of the kernel
     e = d["e2e"]
     assert e["unit"] == d["unit"] and 0 < e["value"] < d["value"] and e["h2d_bytes_per_step"] > 0 < e["d2h_bytes_per_step"]
