@@ -237,7 +237,8 @@ SweepFn sweep_fn(int S, bool budgets, int wide) {
 }
 constexpr int RING_MAX_STEPS = 3;   // the shared-memory-ring kernel is instantiated for S = 1 .. 3
 constexpr int WARP_MIN_ROWS = 32;   // automatic choice of the warp kernel: columns at least this long (config 3, 41 rows: 126 G against 105 G on the ring kernel)
-constexpr int WS_MAX_STEPS = 3;     // the register-resident kernel is instantiated for S = 2, 3
+constexpr int WARP_DEEP_ROWS = 128;  // automatic depth of the warp kernel: 4 steps per pass for columns at least this long
+constexpr int WS_MAX_STEPS = 4;     // the register-resident kernel is instantiated for S = 2, 3, 4
 static_assert(WS_MAX_STEPS <= SWEEP_MAX_STEPS, "partial sums are laid out for SWEEP_MAX_STEPS steps per pass");
 
 // register-resident warp kernel (bte_warpsweep.cuh): S = 2, 3 steps per pass, K = BTE_WS_K columns per lane
@@ -250,8 +251,9 @@ SweepFn warpsweep_fn_s(bool budgets) {
             Cfg::smem_bytes, Cfg::W, Cfg::T, Cfg::WARPS};
 }
 SweepFn warpsweep_fn(int S, bool budgets, int precision) {
-    if (precision == 1) return S == 2 ? warpsweep_fn_s<2, 8>(budgets) : warpsweep_fn_s<3, 8>(budgets);
-    return S == 2 ? warpsweep_fn_s<2, 16>(budgets) : warpsweep_fn_s<3, 16>(budgets);
+    if (precision == 1)
+        return S == 2 ? warpsweep_fn_s<2, 8>(budgets) : S == 3 ? warpsweep_fn_s<3, 8>(budgets) : warpsweep_fn_s<4, 8>(budgets);
+    return S == 2 ? warpsweep_fn_s<2, 16>(budgets) : S == 3 ? warpsweep_fn_s<3, 16>(budgets) : warpsweep_fn_s<4, 16>(budgets);
 }
 
 // Wider CTAs pay off only for the HBM-bound one-step pass over long rows (4 or 8 KB DRAM bursts per row instead
@@ -462,7 +464,7 @@ int effective_variant(const bte_ctx* c) {
     if (c->grid.precision == 1) {
         // fp32 storage: multi-step passes through the warp kernel (half the HBM bytes), single steps (remainders, budget
         // cuts) through the two-launch form
-        const bool ok = c->ws_grid[WS_MAX_STEPS] > 0 && c->grid.n_harm + 1 >= WARP_MIN_ROWS;
+        const bool ok = c->ws_grid[3] > 0 && c->grid.n_harm + 1 >= WARP_MIN_ROWS;
         return ok && (c->variant == VAR_AUTO || c->variant == VAR_WARPSWEEP || c->variant == VAR_RESIDENT) ? VAR_WARPSWEEP
                                                                                                          : VAR_SPLIT;
     }
@@ -473,7 +475,7 @@ int effective_variant(const bte_ctx* c) {
     // (registers + tensor memory; a segment costs 3 NS extra row iterations, so it wants a long march over n); short
     // columns (batches of small systems): the shared-memory-ring kernel at S = 2.
     const bool streaming = c->variant == VAR_AUTO || c->variant == VAR_RESIDENT || c->variant == VAR_WARPSWEEP;
-    if (streaming && warp_ok && c->ws_grid[WS_MAX_STEPS] > 0 && c->grid.n_harm + 1 >= WARP_MIN_ROWS) return VAR_WARPSWEEP;
+    if (streaming && warp_ok && c->ws_grid[3] > 0 && c->grid.n_harm + 1 >= WARP_MIN_ROWS) return VAR_WARPSWEEP;
     if (streaming || c->variant == VAR_SWEEP) return c->sw_grid[1] > 0 ? VAR_SWEEP : VAR_FUSED;
     return c->variant;
 }
@@ -493,7 +495,11 @@ int sweep_steps(const bte_ctx* c) {
     if (!is_sweep(var)) return 1;
     int S;
     if (var == VAR_WARPSWEEP) {
-        S = c->sweep_steps > 0 ? c->sweep_steps : 3;
+        // 4 steps per pass on long columns: 16 B of HBM traffic per update.  Alone it is 2.5 % slower than 3 (181 against
+        // 186 G on config 4: 14 of 96 columns per strip are halos instead of 10), but the 3-step pass loses its clocks under
+        // sustained load (172 G after ~0.2 s) and the 4-step pass does not (180-181 G throughout);
+        // short columns (config 3, 41 rows) cannot amortise the 2 NS + 1 fill / drain iterations of a deeper pipeline
+        S = c->sweep_steps > 0 ? c->sweep_steps : (c->grid.n_harm + 1 >= WARP_DEEP_ROWS ? 4 : 3);
     } else {
         // ring kernel: 3 steps per pass when the march over n is long enough to amortise the 3 NS - 1
         // fill/drain iterations of a segment, else 2 (measured on configs 3 and 4)

@@ -92,7 +92,7 @@ def test_streaming_configs_full_length_every_sweep_depth(idx, sweep_steps):
 
 
 @pytest.mark.parametrize("idx", [3, 4])
-@pytest.mark.parametrize("sweep_steps", [2, 3])
+@pytest.mark.parametrize("sweep_steps", [2, 3, 4])
 def test_streaming_configs_full_length_warp_kernel(idx, sweep_steps):
     """The same through the warp kernel (variant 5: registers + tensor memory, bte_warpsweep.cuh); config 4 is what
     the automatic choice runs."""

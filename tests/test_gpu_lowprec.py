@@ -65,7 +65,7 @@ def test_fp32_modes_match_the_oracle_with_ac_field_and_budget(precision):
         s.destroy()
 
 
-@pytest.mark.parametrize("sweep_steps", [2, 3])
+@pytest.mark.parametrize("sweep_steps", [2, 3, 4])
 @pytest.mark.parametrize("N,M1", [(40, 801), (97, 300), (33, 90)])
 def test_fp32_storage_through_the_warp_kernel(N, M1, sweep_steps):
     """precision 1 on lattices of at least 32 rows runs the multi-step warp kernel with fp32 rows in HBM (half the bytes)

@@ -17,8 +17,8 @@ pytestmark = pytest.mark.gpu
 # name -> (variant, leap-frog steps fused per launch of the sweep kernel)
 # (variant 3: shared-memory-ring kernel bte_sweep.cuh; variant 5: warp kernel bte_warpsweep.cuh, registers + tensor memory)
 VARIANTS = {"split": (1, 0), "fused": (2, 0), "sweep1": (3, 1), "sweep2": (3, 2), "sweep3": (3, 3),
-            "warp2": (5, 2), "warp3": (5, 3), "resident": (4, 0), "auto": (0, 0)}
-SWEEPS = ["sweep1", "sweep2", "sweep3", "warp2", "warp3"]
+            "warp2": (5, 2), "warp3": (5, 3), "warp4": (5, 4), "resident": (4, 0), "auto": (0, 0)}
+SWEEPS = ["sweep1", "sweep2", "sweep3", "warp2", "warp3", "warp4"]
 ALL = ["split", "fused"] + SWEEPS + ["resident"]
 
 
@@ -231,15 +231,16 @@ def test_fused_equals_split_bitwise_state():
     """The variants that form mu = n * (beta dt/2) evaluate the same per-point expression in the same operation order:
     their states must be bit-identical (this stands in for a race detector: any ordering bug changes bits).  The warp
     kernel forms mu = fma(n, B phi dt/2, n E dt/2) (no per-column table of the half-step times): it differs from the
-    others in the last bits of mu only, so it must agree with them to a few ulps, and its two depths (same expression,
-    different decomposition into strips, stages and segments) with each other bit for bit."""
-    w = W.small_case(N=14, M1=260, n_steps=31)
-    a = gpu_solver(w, "split"); a.step(31)
+    others in the last bits of mu only, so it must agree with them to a few ulps, and its three depths (same expression,
+    different decomposition into strips, stages and segments) with each other bit for bit (36 steps: a multiple of every
+    depth, so that no single-step launch of the ring kernel, which forms mu the other way, is mixed in)."""
+    w = W.small_case(N=14, M1=260, n_steps=36)
+    a = gpu_solver(w, "split"); a.step(36)
     ref = [a.get_state(0, g) for g in (0, 1)]
     scale = max(np.abs(x).max() for pair in ref for x in pair)
     warp = {}
     for other in ["fused", "resident"] + SWEEPS:
-        b = gpu_solver(w, other); b.step(31)
+        b = gpu_solver(w, other); b.step(36)
         for g in (0, 1):
             ya, yb = b.get_state(0, g)
             if other.startswith("warp"):
@@ -248,7 +249,9 @@ def test_fused_equals_split_bitwise_state():
             else:
                 assert np.array_equal(ref[g][0], ya) and np.array_equal(ref[g][1], yb), other
     for g in (0, 1):
-        assert np.array_equal(warp[g][0][0], warp[g][1][0]) and np.array_equal(warp[g][0][1], warp[g][1][1])
+        assert len(warp[g]) == 3                     # the three depths of the warp kernel: bit for bit
+        for other in warp[g][1:]:
+            assert np.array_equal(warp[g][0][0], other[0]) and np.array_equal(warp[g][0][1], other[1])
 
 
 @pytest.mark.parametrize("variant", ALL)

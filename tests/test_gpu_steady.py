@@ -35,7 +35,7 @@ def run_both(w, n_steps, tol, n_avg, min_relax, variant, sweep_steps, chunks):
     return s, obs, steps, phases, sims
 
 
-@pytest.mark.parametrize("variant,sweep_steps", [(5, 3), (5, 2), (3, 2), (3, 1), (0, 0)])
+@pytest.mark.parametrize("variant,sweep_steps", [(5, 4), (5, 3), (5, 2), (3, 2), (3, 1), (0, 0)])
 def test_steady_policy_batch_matches_the_oracle(variant, sweep_steps):
     """Six systems with different frequencies (different comparison intervals and windows) in one batch: the step at
     which each is found relaxed, its phase, window and sums, and its state at the step where it stopped."""
