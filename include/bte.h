@@ -30,7 +30,7 @@
  *     time (a cudaStream_t passed as void*; NULL = legacy default stream).
  *   - How a step is executed is chosen automatically (bte_set_option "variant"): lattices that fit the GPU's
  *     shared memory run the whole time loop of a bte_step call in one launch (resident kernel); larger ones and
- *     batches stream through HBM once per 3 time steps (warp kernel; columns shorter than 32 rows: the
+ *     batches stream through HBM once per 4 or 3 time steps (warp kernel; columns shorter than 32 rows: the
  *     shared-memory-ring kernel, 2 steps).  Results do not depend on the choice beyond rounding: the state is
  *     bit-identical across variants 1-4 and agrees with variant 5 to 1e-14 max|f| (variant 5 forms n beta dt/2 with
  *     one fused multiply-add more).
@@ -221,7 +221,7 @@ BTE_API int bte_rs_evolve_static(const bte_rs_grid* grid /* host */, const bte_p
  *                  3 = persistent sweep kernel, S steps per launch (64/S B/point/step; intermediate time levels in
  *                      shared-memory rings, one thread per phi_y column; the one-step, HBM-bound form and the
  *                      default for columns shorter than 32 rows),
- *                  5 = warp kernel, S = 2 or 3 steps per launch (same traffic; the default path for lattices larger
+ *                  5 = warp kernel, S = 2, 3 or 4 steps per launch (same traffic; the default path for lattices larger
  *                      than the GPU's shared memory and for batches: one warp per strip of 96 columns runs all 2 S
  *                      half-updates in registers, rows in flight in tensor memory, input rows by 1-D TMA bulk copies;
  *                      one-step launches fall back to variant 3; also bte_grid.precision 1),
@@ -233,7 +233,7 @@ BTE_API int bte_rs_evolve_static(const bte_rs_grid* grid /* host */, const bte_p
  *                  grid; 0 = automatic
  *   "resident_halo" halo columns per side of a slab in the cooperative-grid mode of variant 4 (1..4): neighbours
  *                  exchange their edge columns once per that many half-updates; 0 = automatic (3)
- *   "sweep_steps"  S of variant 3 (1..3) or 5 (2..3), 0 = automatic
+ *   "sweep_steps"  S of variant 3 (1..3) or 5 (2..4), 0 = automatic (variant 5: 4 for columns of >= 128 rows, else 3)
  *   "sweep_ctas"   CTAs of the persistent sweep kernel, 0 = SMs x resident CTAs
  *   "sweep_threads" threads per CTA of the sweep kernel: 128, 256 or (one-step pass only) 512, 0 = automatic
  *   "graph_steps"  launches captured per CUDA graph for launch-bound grids; 0 = plain launches, -1 = auto

@@ -48,6 +48,7 @@
 #include "bte_sweep.cuh"
 
 // Tuning constants (compile-time; the defaults are the measured optimum on B200, DESIGN.md 5.1a / section 10):
+//   (S = 2, 3, 4 steps per pass are instantiated; bte.cu picks 4 for long columns, else 3)
 //   WARPS 8 (two per SMSP: 254 registers each), K 3 columns per lane, DIN 4 ring slots, CG 3 stages per coefficient
 //   group, COVER 6 (a segment is charged COVER * NS / 2 = 3 NS row-iterations in the partition), TMSLOT 0 = automatic
 #ifndef BTE_WS_WARPS
