@@ -237,7 +237,9 @@ SweepFn sweep_fn(int S, bool budgets, int wide) {
 }
 constexpr int RING_MAX_STEPS = 3;   // the shared-memory-ring kernel is instantiated for S = 1 .. 3
 constexpr int WARP_MIN_ROWS = 32;   // automatic choice of the warp kernel: columns at least this long (config 3, 41 rows: 126 G against 105 G on the ring kernel)
-constexpr int WARP_DEEP_ROWS = 128;  // automatic depth of the warp kernel: 4 steps per pass for columns at least this long
+constexpr int WARP_DEEP_ROWS = 352;  // automatic depth of the warp kernel: 4 steps per pass for columns at least this long
+                                     // (x 32001 points, sustained G updates/s at S = 3 / 4: 256 rows 158 / 154, 320 rows 166 / 164,
+                                     // 384 rows 171 -> 163 / 170, 448 rows 175 -> 166 / 176, 513 rows 172 / 181, 1024 rows 181 / 191)
 constexpr int WS_MAX_STEPS = 4;     // the register-resident kernel is instantiated for S = 2, 3, 4
 static_assert(WS_MAX_STEPS <= SWEEP_MAX_STEPS, "partial sums are laid out for SWEEP_MAX_STEPS steps per pass");
 
