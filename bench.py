@@ -366,7 +366,11 @@ def hbm_roofline(w, updates_per_block, ms, launches, steps, variant, S, peak, pe
             "effective_note": ("temporal blocking: one pass over the state advances steps_per_launch time steps, so "
                                "the one-step-per-pass figure (64 B per update) can exceed the HBM peak; 'achieved' "
                                "counts what a launch really has to move"),
-            "fp64_pipe_frac": fp64_rate / FP64_PEAK_INSTR}
+            "fp64_pipe_frac": fp64_rate / FP64_PEAK_INSTR,
+            "bound_note": ("SURVEY 8(d) counts HBM bytes, so 'bound' stays hbm; a pass of S >= 2 steps moves 64 / S B per "
+                           "update by design and is limited by the fp64 pipe and the issue slots (fp64_pipe_frac; ncu: "
+                           "profiles/r02f, r02c), the HBM-bound form of the same workload is one_step_per_pass")
+            if S >= 2 else None}
 
 
 def alu_roofline(updates_per_block, ms, steps, launches):
