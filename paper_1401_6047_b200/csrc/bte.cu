@@ -474,7 +474,7 @@ int effective_variant(const bte_ctx* c) {
     const bool warp_ok = c->sw_grid[1] > 0 && c->ws_grid[2] > 0;
     if (c->variant == VAR_WARPSWEEP && warp_ok) return VAR_WARPSWEEP;
     // AUTO, and what runs when the resident kernel is not used: a streaming kernel.  Long columns: the warp kernel
-    // (registers + tensor memory; a segment costs 3 NS extra row iterations, so it wants a long march over n); short
+    // (registers + tensor memory; a segment costs about 2 NS extra row iterations, so it wants a long march over n); short
     // columns (batches of small systems): the shared-memory-ring kernel at S = 2.
     const bool streaming = c->variant == VAR_AUTO || c->variant == VAR_RESIDENT || c->variant == VAR_WARPSWEEP;
     if (streaming && warp_ok && c->ws_grid[3] > 0 && c->grid.n_harm + 1 >= WARP_MIN_ROWS) return VAR_WARPSWEEP;

@@ -50,7 +50,7 @@
 // Tuning constants (compile-time; the defaults are the measured optimum on B200, DESIGN.md 5.1a / section 10):
 //   (S = 2, 3, 4 steps per pass are instantiated; bte.cu picks 4 for long columns, else 3)
 //   WARPS 8 (two per SMSP: 254 registers each), K 3 columns per lane, DIN 4 ring slots, CG 3 stages per coefficient
-//   group, COVER 6 (a segment is charged COVER * NS / 2 = 3 NS row-iterations in the partition; S = 4: 16), TMSLOT 0 = automatic
+//   group, COVER 4 (a segment is charged COVER * NS / 2 = 2 NS row-iterations in the partition), TMSLOT 0 = automatic
 #ifndef BTE_WS_WARPS
 #define BTE_WS_WARPS 8
 #endif
@@ -64,7 +64,7 @@
 #define BTE_WS_TMSLOT 0
 #endif
 #ifndef BTE_WS_COVER
-#define BTE_WS_COVER 6
+#define BTE_WS_COVER 4
 #endif
 #ifndef BTE_WS_CG
 #define BTE_WS_CG 3
@@ -587,14 +587,14 @@ __global__ void __launch_bounds__(WarpCfg<S, K, EB>::T, 1) warpsweep_kernel(cons
     asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
 
     // ---- active systems and this CTA's range of band-rows --------------------------------------------
-    // Static partition balanced by COST, not by rows: a segment costs its rows plus about 3 NS row-iterations of
+    // Static partition balanced by COST, not by rows: a segment costs its rows plus about 2 NS row-iterations of
     // pipeline fill / drain and halo rows (slower, predicated iterations), so a range that spans a band boundary must
     // get fewer rows.  Every band is charged c_over + rows cost units; the i-th boundary sits at cost i / gridDim.x
     // of the total (boundaries that fall into a band's overhead snap to the band's first row).
     auto range_cut = [&](const long long i, const long long nb) -> long long {
-        // (measured optimum on config 4: 18 row-iterations at S = 3, 16 at S = 4 -- 12 / 20 / 24 there: 181.5 / 182.6 / 181.5
-        // against 184.3 G: the cost of a segment does not grow with the depth of the pipeline)
-        const long long c_over = S >= 4 ? 16 : BTE_WS_COVER * Cfg::NS / 2, band_cost = rows + c_over;
+        // (c_over = 2 NS, measured: config 4 at S = 4 with 8 / 12 / 16 / 20 / 24 / 32 row-iterations: 181.5 / 184.0 / 184.3 /
+        // 182.6 / 181.5 / 179.2 G; config 3 at S = 3 with 6 / 9 / 12 / 15 / 18 / 21: 132.9 / 133.7 / 136.3 / 135.8 / 135.5 / 134.9 G)
+        const long long c_over = BTE_WS_COVER * Cfg::NS / 2, band_cost = rows + c_over;
         const long long y = (i * nb * band_cost) / gridDim.x;
         const long long b = y / band_cost, r = y - b * band_cost;
         return b * rows + min(max(r - c_over, 0LL), (long long)rows);
