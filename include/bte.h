@@ -233,7 +233,7 @@ BTE_API int bte_rs_evolve_static(const bte_rs_grid* grid /* host */, const bte_p
  *                  grid; 0 = automatic
  *   "resident_halo" halo columns per side of a slab in the cooperative-grid mode of variant 4 (1..4): neighbours
  *                  exchange their edge columns once per that many half-updates; 0 = automatic (3)
- *   "sweep_steps"  S of variant 3 (1..3) or 5 (2..4), 0 = automatic (variant 5: 4 for columns of >= 352 rows, else 3)
+ *   "sweep_steps"  S of variant 3 (1..3) or 5 (2..4), 0 = automatic (variant 5: 4 for columns of >= 320 rows, else 3)
  *   "sweep_ctas"   CTAs of the persistent sweep kernel, 0 = SMs x resident CTAs
  *   "sweep_threads" threads per CTA of the sweep kernel: 128, 256 or (one-step pass only) 512, 0 = automatic
  *   "graph_steps"  launches captured per CUDA graph for launch-bound grids; 0 = plain launches, -1 = auto

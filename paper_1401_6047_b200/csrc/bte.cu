@@ -237,9 +237,10 @@ SweepFn sweep_fn(int S, bool budgets, int wide) {
 }
 constexpr int RING_MAX_STEPS = 3;   // the shared-memory-ring kernel is instantiated for S = 1 .. 3
 constexpr int WARP_MIN_ROWS = 32;   // automatic choice of the warp kernel: columns at least this long (config 3, 41 rows: 126 G against 105 G on the ring kernel)
-constexpr int WARP_DEEP_ROWS = 352;  // automatic depth of the warp kernel: 4 steps per pass for columns at least this long
-                                     // (x 32001 points, sustained G updates/s at S = 3 / 4: 256 rows 158 / 154, 320 rows 166 / 164,
-                                     // 384 rows 171 -> 163 / 170, 448 rows 175 -> 166 / 176, 513 rows 172 / 181, 1024 rows 181 / 191)
+constexpr int WARP_DEEP_ROWS = 320;  // automatic depth of the warp kernel: 4 steps per pass for columns at least this long
+                                     // (x 32001 points, sustained G updates/s over 7200 steps at S = 3 / 4: 256 rows 158 / 154,
+                                     // 288 rows 164 / 162, 320 rows 168 -> 160 / 167, 352 rows 170 -> 160 / 172,
+                                     // 384 rows 172 -> 163 / 173, 513 rows 173 / 184, 1024 rows 181 / 191)
 constexpr int WS_MAX_STEPS = 4;     // the register-resident kernel is instantiated for S = 2, 3, 4
 static_assert(WS_MAX_STEPS <= SWEEP_MAX_STEPS, "partial sums are laid out for SWEEP_MAX_STEPS steps per pass");
 
@@ -497,10 +498,10 @@ int sweep_steps(const bte_ctx* c) {
     if (!is_sweep(var)) return 1;
     int S;
     if (var == VAR_WARPSWEEP) {
-        // 4 steps per pass on long columns: 16 B of HBM traffic per update.  Alone it is 2.5 % slower than 3 (181 against
-        // 186 G on config 4: 14 of 96 columns per strip are halos instead of 10), but the 3-step pass loses its clocks under
-        // sustained load (172 G after ~0.2 s) and the 4-step pass does not (180-181 G throughout);
-        // short columns (config 3, 41 rows) cannot amortise the 2 NS + 1 fill / drain iterations of a deeper pipeline
+        // 4 steps per pass on long columns: 16 B of HBM traffic per update.  Alone it is 2 % slower than 3 (184 against
+        // 188 G on config 4: 14 of 96 columns per strip are halos instead of 10), but the 3-step pass loses its clocks under
+        // sustained load (172-175 G after ~0.2 s) and the 4-step pass does not (183-184.6 G
+        // throughout); shorter columns run too slowly to lose their clocks and pay more for the deeper pipeline
         S = c->sweep_steps > 0 ? c->sweep_steps : (c->grid.n_harm + 1 >= WARP_DEEP_ROWS ? 4 : 3);
     } else {
         // ring kernel: 3 steps per pass when the march over n is long enough to amortise the 3 NS - 1
